@@ -1,0 +1,134 @@
+/*
+ * vox.h -- C ABI of the B200 tetrahedral-mesh -> solid-binary-voxel library.
+ *
+ * What it computes (arxiv 2106.01326; citations are PAPER.md line numbers):
+ *   "voxelizing the tetrahedral mesh according to whether the sampling point is
+ *   within a tetrahedral or not": for every voxel-centre sample P
+ *   of an nx*ny*nz grid and every tet whose bounding box covers P ("We iterate
+ *   over every bounding box of the tetrahedral and apply the ... point-in-
+ *   tetrahedral test") evaluate Theorem 1's four determinants
+ *    and OR the result into a bit grid ("binary 3D grid",
+ *   PAPER.md:110).
+ *
+ * Readings where the paper is silent:
+ *   - the test is INCLUSIVE (closed tets);  tets with 6V == 0 contribute nothing;
+ *   - sample = voxel centre  P = (hx*x + hx/2, hy*y + hy/2, hz*z + hz/2),
+ *     h = extent / n per axis, on the integer lattice;
+ *   - coordinates are int32 lattice points in [0, extent]; all predicates are
+ *     evaluated in exact integer arithmetic (no floating point decides a bit).
+ *
+ * Grid layout (output of vox_run): for mesh m of the batch, voxel (x,y,z)
+ *   word = ((m*nz + z)*ny + y)*(nx/32) + (x >> 5),  bit = x & 31  (LSB = lowest x),
+ *   bit = 1 iff solid.  Every word of the grid is written by every vox_run.
+ *
+ * Memory ownership: ALL device memory is the caller's.  vox_tets borrows the
+ * input pointers (no copy) until the last vox_run using them has completed on
+ * its stream.  Workspace and output are caller-allocated.  The library
+ * allocates only the host-side context.  vox_run only enqueues work on the
+ * given stream: no allocation, no host synchronisation.
+ *
+ * Pointers named d_* are DEVICE pointers, h_* are HOST pointers.
+ * `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *
+ * Errors: every int-returning call returns VOX_OK (0) or a negative code;
+ * nothing aborts or throws across the ABI.
+ */
+#ifndef VOX_H_
+#define VOX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vox_ctx vox_ctx; /* opaque, host side */
+
+enum {
+    VOX_OK = 0,
+    VOX_EINVAL = -1,     /* null pointer, n <= 0, nx % 32 != 0, extent % (2n) != 0, batch < 1, V/T < 0 */
+    VOX_ERANGE = -2,     /* extent > 2^20 (the int64 bound 6*extent^3 < 2^63 would not hold), n > 32768 */
+    VOX_EWORKSPACE = -3, /* workspace too small (at enqueue, or reported by vox_status after a run) */
+    VOX_ECUDA = -4,      /* CUDA runtime error; text via vox_last_error */
+    VOX_ESTATE = -5,     /* call order: vox_run before vox_tets, ... */
+    VOX_EDATA = -6       /* vox_validate: a vertex outside [0,extent] or a tet index outside [0,V) */
+};
+
+/* Grid dims in voxels (nx % 32 == 0), lattice extent per axis (extent % (2n) == 0
+ * so that voxel centres are lattice points; extent <= 2^20), batch >= 1 meshes
+ * sharing the grid shape.  Picks the binning tile (32 x TY x TZ voxels). */
+int vox_create(vox_ctx** out, int nx, int ny, int nz, int ex, int ey, int ez, int batch);
+void vox_destroy(vox_ctx* ctx);
+
+/* Optional: override the binning tile height/depth (powers of two in [4,32]).
+ * Must precede vox_tets.  The result of vox_run does not depend on it. */
+int vox_set_tile(vox_ctx* ctx, int ty, int tz);
+
+/* Optional: kernel variant of the brick voxelizer, 0 = default.  Result-neutral
+ * (used by tests and the benchmark to compare variants). */
+int vox_set_variant(vox_ctx* ctx, int variant);
+
+/* Borrow the mesh.  d_verts int32[V][3] with coordinates in [0, extent];
+ * d_tets int32[T][4], indices global into d_verts; d_tet_offsets int64[batch+1]
+ * (device; mesh m owns tets [off[m], off[m+1]); off[0] = 0, off[batch] = T), or
+ * NULL when batch == 1.  T == 0 is legal (all-zero grid). */
+int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const int32_t* d_tets, int64_t T,
+             const int64_t* d_tet_offsets);
+
+/* batch * nz * ny * (nx/32) */
+size_t vox_grid_words(const vox_ctx* ctx);
+
+/* Workspace vox_run needs.  After vox_tets: the fixed part plus room for an
+ * ESTIMATED number of (tet, brick) pairs (4*T + bricks).  After vox_plan: exact. */
+size_t vox_workspace_bytes(const vox_ctx* ctx);
+/* The part of the workspace that does not depend on the pair count (what vox_plan needs). */
+size_t vox_workspace_fixed_bytes(const vox_ctx* ctx);
+
+/* Optional exact sizing: runs the count + scan passes (K1, K2) on `cuda_stream`,
+ * SYNCHRONISES it, and returns the number of (tet, brick) pairs.  Afterwards
+ * vox_workspace_bytes is exact for this mesh.  Needs ws_bytes >= fixed bytes. */
+int vox_plan(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes, int64_t* pairs_out);
+
+/* Enqueue the whole hot path (K1 count, K2 scan, K3 scatter, K4 brick voxelizer
+ * with its large-tet path) on `cuda_stream`; writes every word of d_bits_out.
+ * If the workspace cannot hold all pairs the excess tets are dropped and a device
+ * flag is raised that vox_status reports. */
+int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes, uint32_t* d_bits_out);
+
+/* SYNCHRONISES the stream and reads the header the last vox_run left in the
+ * workspace: returns VOX_EWORKSPACE if pairs were dropped; stats_out (may be
+ * NULL) receives {pairs, culled tets (sliver or degenerate), large-path pairs,
+ * non-empty bricks}. */
+int vox_status(vox_ctx* ctx, void* cuda_stream, const void* d_workspace, int64_t stats_out[4]);
+
+/* Debug: device pass + sync; VOX_EDATA if a vertex lies outside [0,extent] or a
+ * tet index outside [0,V) or the offsets are not monotone.  d_workspace needs
+ * only the fixed part. */
+int vox_validate(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes);
+
+/* End-to-end convenience for HOST buffers (the call the e2e benchmark times):
+ * copies h_verts / h_tets / h_tet_offsets into the caller's device arena, runs
+ * vox_tets + vox_run on `cuda_stream`, copies the grid to h_bits_out and
+ * synchronises.  Host buffers should be pinned.  Arena layout is private;
+ * vox_host_arena_bytes(ctx, V, T) says how large it must be (it includes an
+ * estimated-pairs workspace; pass a larger arena for pathological meshes).
+ * Returns VOX_EWORKSPACE if pairs were dropped. */
+size_t vox_host_arena_bytes(const vox_ctx* ctx, int64_t V, int64_t T);
+int vox_run_host(vox_ctx* ctx, void* cuda_stream, const int32_t* h_verts, int64_t V,
+                 const int32_t* h_tets, int64_t T, const int64_t* h_tet_offsets,
+                 void* d_arena, size_t arena_bytes, uint32_t* h_bits_out);
+
+/* Roofline probe (not on the hot path): enqueue a dependent-free integer kernel
+ * on `cuda_stream`.  kind 0 = IADD3/LOP3 stream (alu pipe), 1 = IMAD stream
+ * (fma pipe), 2 = mixed.  *ops_out = thread-level INT32 ops it executes. */
+int vox_probe_int32(void* cuda_stream, int kind, int blocks, int iters, uint32_t* d_sink,
+                    double* ops_out);
+
+const char* vox_strerror(int code);
+const char* vox_last_error(const vox_ctx* ctx); /* CUDA error text of the last VOX_ECUDA */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VOX_H_ */

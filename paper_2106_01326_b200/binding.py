@@ -1,0 +1,300 @@
+"""ctypes binding of include/vox.h.  Marshalling only; torch supplies device memory and streams."""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libvox.so")
+_lib = None
+
+# every symbol include/vox.h declares
+EXPORTS = [
+    "vox_create", "vox_destroy", "vox_set_tile", "vox_set_variant", "vox_tets", "vox_grid_words",
+    "vox_workspace_bytes", "vox_workspace_fixed_bytes", "vox_plan", "vox_run", "vox_status",
+    "vox_validate", "vox_host_arena_bytes", "vox_run_host", "vox_probe_int32", "vox_strerror",
+    "vox_last_error",
+]
+
+
+class VoxError(RuntimeError):
+    def __init__(self, code, where, detail=""):
+        self.code = code
+        super().__init__(f"{where}: {_strerror(code)} ({code}){' -- ' + detail if detail else ''}")
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen libvox.so (built by paper_2106_01326_b200.build).  No fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(
+            f"{_LIB_PATH} is missing: run `python -m paper_2106_01326_b200.build` "
+            "(or __graft_entry__.build()).  There is no CPU fallback."
+        )
+    lib = ctypes.CDLL(_LIB_PATH)
+    vp, i32, i64, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_size_t
+    sig = {
+        "vox_create": (i32, [ctypes.POINTER(vp), i32, i32, i32, i32, i32, i32, i32]),
+        "vox_destroy": (None, [vp]),
+        "vox_set_tile": (i32, [vp, i32, i32]),
+        "vox_set_variant": (i32, [vp, i32]),
+        "vox_tets": (i32, [vp, vp, i64, vp, i64, vp]),
+        "vox_grid_words": (sz, [vp]),
+        "vox_workspace_bytes": (sz, [vp]),
+        "vox_workspace_fixed_bytes": (sz, [vp]),
+        "vox_plan": (i32, [vp, vp, vp, sz, ctypes.POINTER(i64)]),
+        "vox_run": (i32, [vp, vp, vp, sz, vp]),
+        "vox_status": (i32, [vp, vp, vp, ctypes.POINTER(i64)]),
+        "vox_validate": (i32, [vp, vp, vp, sz]),
+        "vox_host_arena_bytes": (sz, [vp, i64, i64]),
+        "vox_run_host": (i32, [vp, vp, vp, i64, vp, i64, vp, vp, sz, vp]),
+        "vox_probe_int32": (i32, [vp, i32, i32, i32, vp, ctypes.POINTER(ctypes.c_double)]),
+        "vox_strerror": (ctypes.c_char_p, [i32]),
+        "vox_last_error": (ctypes.c_char_p, [vp]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+def _strerror(code):
+    try:
+        return load_library().vox_strerror(code).decode()
+    except Exception:  # pragma: no cover
+        return "error"
+
+
+def _torch_cuda():
+    import torch
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2106_01326_b200 needs a CUDA device: there is no CPU fallback")
+    return torch
+
+
+def _stream_ptr(torch, stream):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+class Voxelizer:
+    """vox_create / vox_tets / vox_run with torch tensors as device memory.
+
+    verts int32[V][3], tets int32[T][4] and tet_offsets int64[batch+1] are CUDA
+    tensors borrowed by the library; run() returns a uint32-as-int32 CUDA tensor
+    of shape [batch][nz][ny][nx/32] (layout: include/vox.h).
+    """
+
+    def __init__(self, grid, extent=(65536, 65536, 65536), batch=1, tile=None, variant=0):
+        self._lib = load_library()
+        self._ctx = ctypes.c_void_p()
+        self.grid = tuple(int(g) for g in grid)
+        self.extent = tuple(int(e) for e in extent)
+        self.batch = int(batch)
+        rc = self._lib.vox_create(ctypes.byref(self._ctx), *self.grid, *self.extent, self.batch)
+        if rc:
+            raise VoxError(rc, "vox_create")
+        if tile is not None:
+            self._ck(self._lib.vox_set_tile(self._ctx, int(tile[0]), int(tile[1])), "vox_set_tile")
+        if variant:
+            self._ck(self._lib.vox_set_variant(self._ctx, int(variant)), "vox_set_variant")
+        self._keep = None
+        self._ws = None
+        self._out = None
+
+    def _ck(self, rc, where):
+        if rc:
+            raise VoxError(rc, where, self._lib.vox_last_error(self._ctx).decode())
+
+    def close(self):
+        if self._ctx:
+            self._lib.vox_destroy(self._ctx)
+            self._ctx = ctypes.c_void_p()
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def grid_words(self):
+        return int(self._lib.vox_grid_words(self._ctx))
+
+    @property
+    def workspace_bytes(self):
+        return int(self._lib.vox_workspace_bytes(self._ctx))
+
+    @property
+    def workspace_fixed_bytes(self):
+        return int(self._lib.vox_workspace_fixed_bytes(self._ctx))
+
+    def set_tets(self, verts, tets, tet_offsets=None):
+        torch = _torch_cuda()
+        assert verts.is_cuda and tets.is_cuda and verts.dtype == torch.int32 and tets.dtype == torch.int32
+        assert verts.is_contiguous() and tets.is_contiguous()
+        V = verts.numel() // 3
+        T = tets.numel() // 4
+        off_ptr = None
+        if self.batch > 1:
+            assert tet_offsets is not None and tet_offsets.is_cuda and tet_offsets.dtype == torch.int64
+            assert tet_offsets.numel() == self.batch + 1 and tet_offsets.is_contiguous()
+            off_ptr = ctypes.c_void_p(tet_offsets.data_ptr())
+        self._ck(
+            self._lib.vox_tets(self._ctx, ctypes.c_void_p(verts.data_ptr()), V,
+                               ctypes.c_void_p(tets.data_ptr()), T, off_ptr),
+            "vox_tets",
+        )
+        self._keep = (verts, tets, tet_offsets)
+        self.T, self.V = T, V
+
+    def alloc_workspace(self, nbytes=None):
+        torch = _torch_cuda()
+        n = int(nbytes if nbytes is not None else self.workspace_bytes)
+        self._ws = torch.empty(max(n, 256), dtype=torch.uint8, device="cuda")
+        return self._ws
+
+    def plan(self, stream=None):
+        """Exact workspace sizing (count + scan pre-pass; synchronises).  Returns the pair count."""
+        torch = _torch_cuda()
+        if self._ws is None or self._ws.numel() < self.workspace_fixed_bytes:
+            self.alloc_workspace(self.workspace_fixed_bytes)
+        pairs = ctypes.c_int64(0)
+        self._ck(
+            self._lib.vox_plan(self._ctx, _stream_ptr(torch, stream), ctypes.c_void_p(self._ws.data_ptr()),
+                               self._ws.numel(), ctypes.byref(pairs)),
+            "vox_plan",
+        )
+        if self._ws.numel() < self.workspace_bytes:
+            self.alloc_workspace()
+        return int(pairs.value)
+
+    def run(self, out=None, stream=None):
+        torch = _torch_cuda()
+        if self._ws is None:
+            self.alloc_workspace()
+        if out is None:
+            nx, ny, nz = self.grid
+            out = torch.empty((self.batch, nz, ny, nx // 32), dtype=torch.int32, device="cuda")
+        assert out.is_cuda and out.is_contiguous() and out.numel() == self.grid_words
+        self._ck(
+            self._lib.vox_run(self._ctx, _stream_ptr(torch, stream), ctypes.c_void_p(self._ws.data_ptr()),
+                              self._ws.numel(), ctypes.c_void_p(out.data_ptr())),
+            "vox_run",
+        )
+        return out
+
+    def status(self, stream=None):
+        """Synchronises.  Returns dict(pairs, culled, large_pairs, nonempty_tiles); raises on overflow."""
+        torch = _torch_cuda()
+        st = (ctypes.c_int64 * 4)()
+        rc = self._lib.vox_status(self._ctx, _stream_ptr(torch, stream), ctypes.c_void_p(self._ws.data_ptr()), st)
+        self._ck(rc, "vox_status")
+        return dict(pairs=int(st[0]), culled=int(st[1]), large_pairs=int(st[2]), nonempty_tiles=int(st[3]))
+
+    def validate(self, stream=None):
+        torch = _torch_cuda()
+        if self._ws is None:
+            self.alloc_workspace()
+        self._ck(
+            self._lib.vox_validate(self._ctx, _stream_ptr(torch, stream), ctypes.c_void_p(self._ws.data_ptr()),
+                                   self._ws.numel()),
+            "vox_validate",
+        )
+
+    # -- host-buffer end-to-end path (vox_run_host) ---------------------------------------
+    def host_arena_bytes(self, V, T):
+        return int(self._lib.vox_host_arena_bytes(self._ctx, int(V), int(T)))
+
+    def run_host(self, h_verts, h_tets, h_out, arena, h_tet_offsets=None, stream=None):
+        """h_* are (pinned) CPU tensors; arena is a CUDA uint8 tensor.  Synchronises."""
+        torch = _torch_cuda()
+        V = h_verts.numel() // 3
+        T = h_tets.numel() // 4
+        off_ptr = ctypes.c_void_p(h_tet_offsets.data_ptr()) if h_tet_offsets is not None else None
+        self._ck(
+            self._lib.vox_run_host(self._ctx, _stream_ptr(torch, stream), ctypes.c_void_p(h_verts.data_ptr()), V,
+                                   ctypes.c_void_p(h_tets.data_ptr()), T, off_ptr,
+                                   ctypes.c_void_p(arena.data_ptr()), arena.numel(),
+                                   ctypes.c_void_p(h_out.data_ptr())),
+            "vox_run_host",
+        )
+        return h_out
+
+
+def voxelize(verts, tets, grid, extent=(65536, 65536, 65536), tet_offsets=None, tile=None, variant=0, exact_plan=True):
+    """One-shot: numpy/torch in, numpy uint32[batch][nz][ny][nx/32] out (device path, via vox_run)."""
+    torch = _torch_cuda()
+    import numpy as np
+
+    def dev(a, dt):
+        if isinstance(a, torch.Tensor):
+            return a.to(device="cuda", dtype=dt).contiguous()
+        return torch.from_numpy(np.ascontiguousarray(a)).to(device="cuda", dtype=dt).contiguous()
+
+    v = dev(verts, torch.int32).reshape(-1, 3)
+    t = dev(tets, torch.int32).reshape(-1, 4)
+    batch = 1 if tet_offsets is None else len(tet_offsets) - 1
+    off = dev(tet_offsets, torch.int64) if tet_offsets is not None else None
+    vz = Voxelizer(grid, extent, batch, tile=tile, variant=variant)
+    try:
+        vz.set_tets(v, t, off)
+        if exact_plan:
+            vz.plan()
+        out = vz.run()
+        vz.last_status = vz.status()
+        res = out.cpu().numpy().view(np.uint32)
+        voxelize.last_status = vz.last_status
+        return res
+    finally:
+        vz.close()
+
+
+def voxelize_host(verts, tets, grid, extent=(65536, 65536, 65536), tet_offsets=None):
+    """One-shot through vox_run_host (host buffers in, host grid out)."""
+    torch = _torch_cuda()
+    import numpy as np
+
+    hv = torch.from_numpy(np.ascontiguousarray(verts, dtype=np.int32)).pin_memory()
+    ht = torch.from_numpy(np.ascontiguousarray(tets, dtype=np.int32)).pin_memory()
+    batch = 1 if tet_offsets is None else len(tet_offsets) - 1
+    ho = torch.from_numpy(np.ascontiguousarray(tet_offsets, dtype=np.int64)).pin_memory() if batch > 1 else None
+    vz = Voxelizer(grid, extent, batch)
+    try:
+        nx, ny, nz = vz.grid
+        out = torch.empty((batch, nz, ny, nx // 32), dtype=torch.int32).pin_memory()
+        arena = torch.empty(vz.host_arena_bytes(hv.numel() // 3, ht.numel() // 4), dtype=torch.uint8, device="cuda")
+        vz.run_host(hv, ht, out, arena, ho)
+        return out.numpy().view(np.uint32)
+    finally:
+        vz.close()
+
+
+def probe_int32(kind=0, blocks=148 * 16, iters=4096, repeats=5):
+    """Measured INT32 throughput (thread-ops/s) of the probe kernel; CUDA events on the current stream."""
+    torch = _torch_cuda()
+    lib = load_library()
+    sink = torch.zeros(4, dtype=torch.int32, device="cuda")
+    ops = ctypes.c_double(0)
+    st = _stream_ptr(torch, None)
+    best = None
+    for _ in range(repeats + 1):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        rc = lib.vox_probe_int32(st, kind, blocks, iters, ctypes.c_void_p(sink.data_ptr()), ctypes.byref(ops))
+        if rc:
+            raise VoxError(rc, "vox_probe_int32")
+        e1.record()
+        e1.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None else min(best, ms)
+    return ops.value / (best * 1e-3)

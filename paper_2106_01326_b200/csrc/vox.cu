@@ -1,0 +1,829 @@
+// vox.cu -- B200 (sm_100a) tetrahedral-mesh -> solid-binary-voxel hot path.
+//
+// Kernels:
+//   K1 k1_count    per-tet voxel bbox -> tile range, sliver/degenerate cull, per-tile histogram
+//   K2 k2_scan     exclusive scan of the tile counts (+ cursors, totals)
+//   K3 k3_scatter  tet ids into per-tile lists
+//   K4 k4_brick    one CTA per 32 x TY x TZ tile: exact integer edge functions of
+//                  Theorem 1 stepped along rows, row words formed on
+//                  chip, tile image stored once (no global atomics on the grid)
+//   K5 (inside K4) large-tet path: exact tile classification + 64-bit ballot rasteriser
+//
+// Exactness: inside(P) <=> four affine functions G_k(P) >= 0, each an exact integer
+// (DESIGN.md "Arithmetic").  No floating point decides a bit.
+#include "../../include/vox.h"
+
+#include <cuda_runtime.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+typedef long long i64;
+typedef unsigned long long u64;
+typedef unsigned int u32;
+
+// ------------------------------------------------------------------------------------------
+// host context
+// ------------------------------------------------------------------------------------------
+struct Params {
+    const int32_t* verts;
+    const int4* tets;
+    const i64* off;  // device, [batch+1] or NULL
+    i64 T;
+    i64 V;
+    int batch;
+    int nx, ny, nz;
+    int hx, hy, hz;      // pitch per axis
+    int g, g_shift;      // gcd of the pitches; log2(g) or -1
+    int sx, sy, sz;      // h / g
+    int ty_log, tz_log;  // tile = 32 x (1<<ty_log) x (1<<tz_log) voxels
+    int nbx, nby, nbz;   // tiles per axis
+    int wpr;             // words per grid row = nx/32
+    u32 NB;              // tiles in the batch
+    u32 cap;             // capacity of the pair list
+    int ex, ey, ez;
+};
+
+struct vox_ctx {
+    Params p;
+    bool have_tets;
+    i64 pairs_planned;  // -1 = unknown
+    int variant;
+    char err[256];
+};
+
+enum { HDR_WORDS = 64 };
+// header words
+enum { H_TOTAL = 0, H_OVERFLOW = 1, H_CULLED = 2, H_LARGE = 3, H_NONEMPTY = 4, H_BAD = 5, H_TOTAL_HI = 6 };
+
+static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct WsLayout {
+    size_t hdr, counts, cursor, range, list, fixed_end;
+};
+static WsLayout ws_layout(const Params& p) {
+    WsLayout L;
+    size_t o = 0;
+    L.hdr = o;
+    o = align256(o + HDR_WORDS * 4);
+    L.counts = o;
+    o = align256(o + ((size_t)p.NB + 1) * 4);
+    L.cursor = o;
+    o = align256(o + ((size_t)p.NB + 1) * 4);
+    L.range = o;
+    o = align256(o + (size_t)(p.T > 0 ? p.T : 1) * 8);
+    L.list = o;
+    L.fixed_end = o;
+    return L;
+}
+
+// ------------------------------------------------------------------------------------------
+// device helpers: integer geometry
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int floor_div_i(int a, int b) {  // b > 0
+    int q = a / b;
+    int r = a - q * b;
+    return (r < 0) ? q - 1 : q;
+}
+__device__ __forceinline__ i64 floor_div_l(i64 a, i64 b) {  // b > 0
+    i64 q = a / b;
+    i64 r = a - q * b;
+    return (r < 0) ? q - 1 : q;
+}
+
+struct Tet {
+    int ax, ay, az, bx, by, bz, cx, cy, cz, dx, dy, dz;
+};
+
+__device__ __forceinline__ Tet load_tet(const Params& p, i64 t) {
+    int4 id = __ldg(p.tets + t);
+    const int32_t* v = p.verts;
+    Tet q;
+    q.ax = __ldg(v + 3 * (i64)id.x); q.ay = __ldg(v + 3 * (i64)id.x + 1); q.az = __ldg(v + 3 * (i64)id.x + 2);
+    q.bx = __ldg(v + 3 * (i64)id.y); q.by = __ldg(v + 3 * (i64)id.y + 1); q.bz = __ldg(v + 3 * (i64)id.y + 2);
+    q.cx = __ldg(v + 3 * (i64)id.z); q.cy = __ldg(v + 3 * (i64)id.z + 1); q.cz = __ldg(v + 3 * (i64)id.z + 2);
+    q.dx = __ldg(v + 3 * (i64)id.w); q.dy = __ldg(v + 3 * (i64)id.w + 1); q.dz = __ldg(v + 3 * (i64)id.w + 2);
+    return q;
+}
+
+// 6V = det[B-A; C-A; D-A]  (Lemma 1.1)
+__device__ __forceinline__ i64 six_volume(const Tet& q) {
+    i64 ux = q.bx - q.ax, uy = q.by - q.ay, uz = q.bz - q.az;
+    i64 vx = q.cx - q.ax, vy = q.cy - q.ay, vz = q.cz - q.az;
+    i64 wx = q.dx - q.ax, wy = q.dy - q.ay, wz = q.dz - q.az;
+    return ux * (vy * wz - vz * wy) - uy * (vx * wz - vz * wx) + uz * (vx * wy - vy * wx);
+}
+
+// closed voxel-index range of centres h*i + h/2 inside [lo, hi], clamped to the grid
+__device__ __forceinline__ void axis_range(int a, int b, int c, int d, int h, int n, int& i0, int& i1) {
+    int lo = min(min(a, b), min(c, d));
+    int hi = max(max(a, b), max(c, d));
+    i0 = -floor_div_i(h - 2 * lo, 2 * h);  // ceil((2lo - h) / 2h)
+    i1 = floor_div_i(2 * hi - h, 2 * h);
+    i0 = max(i0, 0);
+    i1 = min(i1, n - 1);
+}
+
+__device__ __forceinline__ int mesh_of(const Params& p, i64 t) {
+    if (p.batch == 1) return 0;
+    int lo = 0, hi = p.batch;  // off[lo] <= t < off[hi]
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (__ldg(p.off + mid) <= t) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// ------------------------------------------------------------------------------------------
+// K1: per-tet voxel bbox -> tile range, cull, histogram
+// ------------------------------------------------------------------------------------------
+#define RANGE_CULLED 0xFFFFFFFFu
+
+__global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ range, u32* __restrict__ counts,
+                                                u32* __restrict__ hdr) {
+    i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    bool live = false;
+    uint2 r = make_uint2(RANGE_CULLED, 0u);
+    int m = 0;
+    int b0x = 0, b1x = -1, b0y = 0, b1y = -1, b0z = 0, b1z = -1;
+    if (t < p.T) {
+        Tet q = load_tet(p, t);
+        int x0, x1, y0, y1, z0, z1;
+        axis_range(q.ax, q.bx, q.cx, q.dx, p.hx, p.nx, x0, x1);
+        axis_range(q.ay, q.by, q.cy, q.dy, p.hy, p.ny, y0, y1);
+        axis_range(q.az, q.bz, q.cz, q.dz, p.hz, p.nz, z0, z1);
+        live = (x0 <= x1) && (y0 <= y1) && (z0 <= z1) && (six_volume(q) != 0);
+        if (live) {
+            b0x = x0 >> 5; b1x = x1 >> 5;
+            b0y = y0 >> p.ty_log; b1y = y1 >> p.ty_log;
+            b0z = z0 >> p.tz_log; b1z = z1 >> p.tz_log;
+            r.x = (u32)b0x | ((u32)b0y << 10) | ((u32)b0z << 20);
+            r.y = (u32)b1x | ((u32)b1y << 10) | ((u32)b1z << 20);
+            m = mesh_of(p, t);
+        }
+        range[t] = r;
+    }
+    unsigned dead = __ballot_sync(0xFFFFFFFFu, (t < p.T) && !live);
+    if ((threadIdx.x & 31) == 0 && dead) atomicAdd(hdr + H_CULLED, __popc(dead));
+    if (live) {
+        for (int bz = b0z; bz <= b1z; ++bz)
+            for (int by = b0y; by <= b1y; ++by) {
+                u32 base = (((u32)m * p.nbz + bz) * p.nby + by) * p.nbx;
+                for (int bx = b0x; bx <= b1x; ++bx) atomicAdd(counts + base + bx, 1u);
+            }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// K2: exclusive scan of counts[0..NB) (single CTA; NB is at most a few 10^5)
+// counts[b] <- offset, counts[NB] <- total, cursor[b] <- offset
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) k2_scan(u32 NB, u32* __restrict__ counts, u32* __restrict__ cursor,
+                                                u32* __restrict__ hdr) {
+    __shared__ u64 s_part[1024];
+    __shared__ u32 s_ne[32];
+    const int tid = threadIdx.x;
+    const u32 per = (NB + 1023u) / 1024u;
+    const u32 beg = min(NB, (u32)tid * per), end = min(NB, beg + per);
+    u64 sum = 0;
+    u32 ne = 0;
+    for (u32 i = beg; i < end; ++i) {
+        u32 c = counts[i];
+        sum += c;
+        ne += (c != 0);
+    }
+    s_part[tid] = sum;
+    // non-empty tiles: warp reduce then smem
+    for (int o = 16; o; o >>= 1) ne += __shfl_xor_sync(0xFFFFFFFFu, ne, o);
+    if ((tid & 31) == 0) s_ne[tid >> 5] = ne;
+    __syncthreads();
+    // Hillis-Steele inclusive scan over 1024 partials
+    for (int o = 1; o < 1024; o <<= 1) {
+        u64 v = (tid >= o) ? s_part[tid - o] : 0;
+        __syncthreads();
+        s_part[tid] += v;
+        __syncthreads();
+    }
+    u64 run = s_part[tid] - sum;  // exclusive
+    for (u32 i = beg; i < end; ++i) {
+        u32 c = counts[i];
+        counts[i] = (u32)run;
+        cursor[i] = (u32)run;
+        run += c;
+    }
+    if (tid == 1023) {
+        u64 total = s_part[1023];
+        counts[NB] = (u32)min(total, (u64)0xFFFFFFFFu);
+        hdr[H_TOTAL] = (u32)total;
+        hdr[H_TOTAL_HI] = (u32)(total >> 32);
+        if (total > 0xFFFFFFFFull) hdr[H_OVERFLOW] = 1;
+    }
+    if (tid == 0) {
+        u32 s = 0;
+        for (int i = 0; i < 32; ++i) s += s_ne[i];
+        hdr[H_NONEMPTY] = s;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// K3: scatter tet ids into the per-tile lists
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k3_scatter(Params p, const uint2* __restrict__ range, u32* __restrict__ cursor,
+                                                  u32* __restrict__ list, u32* __restrict__ hdr) {
+    i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= p.T) return;
+    uint2 r = range[t];
+    if (r.x == RANGE_CULLED) return;
+    int b0x = r.x & 1023, b0y = (r.x >> 10) & 1023, b0z = (r.x >> 20) & 1023;
+    int b1x = r.y & 1023, b1y = (r.y >> 10) & 1023, b1z = (r.y >> 20) & 1023;
+    int m = mesh_of(p, t);
+    for (int bz = b0z; bz <= b1z; ++bz)
+        for (int by = b0y; by <= b1y; ++by) {
+            u32 base = (((u32)m * p.nbz + bz) * p.nby + by) * p.nbx;
+            for (int bx = b0x; bx <= b1x; ++bx) {
+                u32 pos = atomicAdd(cursor + base + bx, 1u);
+                if (pos < p.cap) list[pos] = (u32)t;
+                else hdr[H_OVERFLOW] = 1;
+            }
+        }
+}
+
+// ------------------------------------------------------------------------------------------
+// K4: tile voxelizer
+// ------------------------------------------------------------------------------------------
+// The four half-spaces of a non-degenerate tet, written on tile-local voxel indices j:
+//   inside(j) <=> G_k(j) = g0[k] + mx[k]*jx + my[k]*jy + mz[k]*jz >= 0,  k = 0..3.
+// Derivation: Theorem 1's determinants are affine in P:
+//   D_a = N_a.(B-P), N_a=(C-B)x(D-B);  D_b = N_b.(A-P), N_b=(C-A)x(D-A);
+//   D_c = N_c.(A-P), N_c=(B-A)x(D-A);  D_d = N_d.(A-P), N_d=(B-A)x(C-A);
+// with s = sign(6V): inside <=> s*D_a >= 0, -s*D_b >= 0, s*D_c >= 0, -s*D_d >= 0.
+// P = h*(i0+j) + h/2 (componentwise), g = gcd(h): sigma*N.(Q-P) = C - g * sum_a (sigma*N_a*h_a/g) j_a
+// with C = sigma*N.(Q-P0) and the j-sum an integer, so  >= 0  <=>  floor(C/g) - sum >= 0.
+struct Planes {
+    i64 mx[4], my[4], mz[4], g0[4];
+};
+
+__device__ __forceinline__ void one_plane(const Params& p, int k, Planes& P, i64 sig, i64 px, i64 py, i64 pz,
+                                          i64 qx, i64 qy, i64 qz,  // N = p x q
+                                          i64 rx, i64 ry, i64 rz)  // Q - P0
+{
+    i64 nx = sig * (py * qz - pz * qy);
+    i64 ny = sig * (pz * qx - px * qz);
+    i64 nz = sig * (px * qy - py * qx);
+    i64 C = nx * rx + ny * ry + nz * rz;
+    P.mx[k] = -nx * p.sx;
+    P.my[k] = -ny * p.sy;
+    P.mz[k] = -nz * p.sz;
+    P.g0[k] = (p.g_shift >= 0) ? (C >> p.g_shift) : floor_div_l(C, (i64)p.g);
+}
+
+// X0,Y0,Z0: voxel index of the tile origin
+__device__ __forceinline__ void tet_planes(const Params& p, const Tet& q, int X0, int Y0, int Z0, Planes& P) {
+    i64 ux = q.bx - q.ax, uy = q.by - q.ay, uz = q.bz - q.az;
+    i64 vx = q.cx - q.ax, vy = q.cy - q.ay, vz = q.cz - q.az;
+    i64 wx = q.dx - q.ax, wy = q.dy - q.ay, wz = q.dz - q.az;
+    i64 det = ux * (vy * wz - vz * wy) - uy * (vx * wz - vz * wx) + uz * (vx * wy - vy * wx);
+    i64 s = (det > 0) ? 1 : -1;
+    // P0 = centre of the tile-origin voxel
+    i64 p0x = (i64)p.hx * X0 + (p.hx >> 1), p0y = (i64)p.hy * Y0 + (p.hy >> 1), p0z = (i64)p.hz * Z0 + (p.hz >> 1);
+    i64 arx = q.ax - p0x, ary = q.ay - p0y, arz = q.az - p0z;
+    i64 brx = q.bx - p0x, bry = q.by - p0y, brz = q.bz - p0z;
+    // k=0: s * ((C-B)x(D-B)) . (B-P)
+    one_plane(p, 0, P, s, vx - ux, vy - uy, vz - uz, wx - ux, wy - uy, wz - uz, brx, bry, brz);
+    // k=1: -s * ((C-A)x(D-A)) . (A-P)
+    one_plane(p, 1, P, -s, vx, vy, vz, wx, wy, wz, arx, ary, arz);
+    // k=2: s * ((B-A)x(D-A)) . (A-P)
+    one_plane(p, 2, P, s, ux, uy, uz, wx, wy, wz, arx, ary, arz);
+    // k=3: -s * ((B-A)x(C-A)) . (A-P)
+    one_plane(p, 3, P, -s, ux, uy, uz, vx, vy, vz, arx, ary, arz);
+}
+
+__device__ __forceinline__ i64 iabs64(i64 v) { return v < 0 ? -v : v; }
+
+// smem image index of tile row (y,z); skewed so that a tet's rows spread over banks
+__device__ __forceinline__ int img_idx(int y, int z, int ty_log) {
+    return (z << ty_log) + ((y + 11 * z) & ((1 << ty_log) - 1));
+}
+
+enum { REC_W = 18, KIND_FAST = 0, KIND_LARGE = 1 };
+// record: [0..3] mx, [4..7] my, [8..11] mz, [12..15] g0, [16] box, [17] kind | (for LARGE: [0] = tet id)
+
+__device__ __forceinline__ u32 pack_box(int x0, int x1, int y0, int y1, int z0, int z1) {
+    return (u32)x0 | ((u32)x1 << 5) | ((u32)y0 << 10) | ((u32)y1 << 15) | ((u32)z0 << 20) | ((u32)z1 << 25);
+}
+
+// local (tile-relative) closed box of the tet's voxel bbox, intersected with the tile
+__device__ __forceinline__ u32 local_box(const Params& p, const Tet& q, int X0, int Y0, int Z0) {
+    int x0, x1, y0, y1, z0, z1;
+    axis_range(q.ax, q.bx, q.cx, q.dx, p.hx, p.nx, x0, x1);
+    axis_range(q.ay, q.by, q.cy, q.dy, p.hy, p.ny, y0, y1);
+    axis_range(q.az, q.bz, q.cz, q.dz, p.hz, p.nz, z0, z1);
+    const int TY = 1 << p.ty_log, TZ = 1 << p.tz_log;
+    x0 = max(x0 - X0, 0); x1 = min(x1 - X0, 31);
+    y0 = max(y0 - Y0, 0); y1 = min(y1 - Y0, TY - 1);
+    z0 = max(z0 - Z0, 0); z1 = min(z1 - Z0, TZ - 1);
+    return pack_box(x0, x1, y0, y1, z0, z1);
+}
+
+// thread-per-tet setup: writes the record
+__device__ __forceinline__ void setup_record(const Params& p, u32 t, int X0, int Y0, int Z0, int* rec) {
+    Tet q = load_tet(p, t);
+    Planes P;
+    tet_planes(p, q, X0, Y0, Z0, P);
+    u32 box = local_box(p, q, X0, Y0, Z0);
+    bool fits = true;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        i64 bound = iabs64(P.g0[k]) + 31 * (iabs64(P.mx[k]) + iabs64(P.my[k]) + iabs64(P.mz[k]));
+        fits = fits && (bound < 0x7FFFFFFFll);
+    }
+    if (fits) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            rec[k] = (int)P.mx[k];
+            rec[4 + k] = (int)P.my[k];
+            rec[8 + k] = (int)P.mz[k];
+            rec[12 + k] = (int)P.g0[k];
+        }
+        rec[17] = KIND_FAST;
+    } else {
+        rec[0] = (int)t;
+        rec[17] = KIND_LARGE;
+    }
+    rec[16] = (int)box;
+}
+
+// Fast path: all four G fit int32 over the whole tile.  Lanes = rows (y,z) of the
+// tet's local box; each lane walks its row's x-span and builds the row word.
+__device__ __forceinline__ void raster_fast(const int* rec, u32* img, int lane, int ty_log) {
+    const u32 box = (u32)rec[16];
+    const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
+    const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
+    const int w = x1 - x0 + 1, ny = y1 - y0 + 1, nrows = ny * (z1 - z0 + 1);
+    const int n4 = (w + 3) & ~3;  // samples walked: x0+n4-1 down to x0
+    const int4 MX = *reinterpret_cast<const int4*>(rec);
+    const int4 MY = *reinterpret_cast<const int4*>(rec + 4);
+    const int4 MZ = *reinterpret_cast<const int4*>(rec + 8);
+    const int4 G0 = *reinterpret_cast<const int4*>(rec + 12);
+    const int xs = x0 + n4 - 1;
+    // unsigned arithmetic: positions beyond x=31 may wrap; their bits are masked off below
+    const u32 e0 = (u32)G0.x + (u32)MX.x * (u32)xs, e1 = (u32)G0.y + (u32)MX.y * (u32)xs;
+    const u32 e2 = (u32)G0.z + (u32)MX.z * (u32)xs, e3 = (u32)G0.w + (u32)MX.w * (u32)xs;
+    const u32 wmask = 0xFFFFFFFFu >> (32 - w);
+    const u32 inv = (65536u + ny - 1) / ny;  // r / ny for r < 1024, ny <= 32 (checked in tests)
+    for (int r = lane; r < nrows; r += 32) {
+        const int zz = (int)(((u32)r * inv) >> 16);
+        const int y = y0 + (r - zz * ny), z = z0 + zz;
+        u32 r0 = e0 + (u32)MY.x * (u32)y + (u32)MZ.x * (u32)z;
+        u32 r1 = e1 + (u32)MY.y * (u32)y + (u32)MZ.y * (u32)z;
+        u32 r2 = e2 + (u32)MY.z * (u32)y + (u32)MZ.z * (u32)z;
+        u32 r3 = e3 + (u32)MY.w * (u32)y + (u32)MZ.w * (u32)z;
+        u32 out = 0;  // bit q = 1 iff sample x0+q is OUTSIDE
+        for (int i = 0; i < n4; i += 4) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                out = __funnelshift_l(r0 | r1 | r2 | r3, out, 1);
+                r0 -= (u32)MX.x; r1 -= (u32)MX.y; r2 -= (u32)MX.z; r3 -= (u32)MX.w;
+            }
+        }
+        const u32 word = (~out & wmask) << x0;
+        if (word) atomicOr(img + img_idx(y, z, ty_log), word);
+    }
+}
+
+// Large path (K5): planes do not fit int32 on this tile.  The whole warp works on one
+// (tet, tile): exact classification of the local box, then a 64-bit ballot rasteriser
+// with lanes = the 32 x positions of a row word.
+__device__ __noinline__ void raster_large(const Params& p, u32 t, u32 box, int X0, int Y0, int Z0, u32* img, int lane) {
+    Tet q = load_tet(p, t);
+    Planes P;
+    tet_planes(p, q, X0, Y0, Z0, P);
+    const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
+    const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
+    bool all_in = true, any_out = false;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        i64 ax0 = P.mx[k] * x0, ax1 = P.mx[k] * x1, ay0 = P.my[k] * y0, ay1 = P.my[k] * y1;
+        i64 az0 = P.mz[k] * z0, az1 = P.mz[k] * z1;
+        i64 lo = P.g0[k] + min(ax0, ax1) + min(ay0, ay1) + min(az0, az1);
+        i64 hi = P.g0[k] + max(ax0, ax1) + max(ay0, ay1) + max(az0, az1);
+        all_in = all_in && (lo >= 0);
+        any_out = any_out || (hi < 0);
+    }
+    if (any_out) return;  // one half-space misses the whole box: exact, G is affine
+    const u32 xmask = (0xFFFFFFFFu >> (31 - x1 + x0)) << x0;
+    const int ny = y1 - y0 + 1;
+    if (all_in) {  // the box lies inside the tet
+        const int nrows = ny * (z1 - z0 + 1);
+        for (int r = lane; r < nrows; r += 32) {
+            int zz = r / ny;
+            atomicOr(img + img_idx(y0 + r - zz * ny, z0 + zz, p.ty_log), xmask);
+        }
+        return;
+    }
+    i64 c0 = P.g0[0] + P.mx[0] * lane, c1 = P.g0[1] + P.mx[1] * lane;
+    i64 c2 = P.g0[2] + P.mx[2] * lane, c3 = P.g0[3] + P.mx[3] * lane;
+    for (int z = z0; z <= z1; ++z) {
+        i64 r0 = c0 + P.mz[0] * z + P.my[0] * y0, r1 = c1 + P.mz[1] * z + P.my[1] * y0;
+        i64 r2 = c2 + P.mz[2] * z + P.my[2] * y0, r3 = c3 + P.mz[3] * z + P.my[3] * y0;
+        for (int y = y0; y <= y1; ++y) {
+            u32 word = __ballot_sync(0xFFFFFFFFu, (r0 | r1 | r2 | r3) >= 0) & xmask;
+            if (lane == 0 && word) atomicOr(img + img_idx(y, z, p.ty_log), word);
+            r0 += P.my[0]; r1 += P.my[1]; r2 += P.my[2]; r3 += P.my[3];
+        }
+    }
+}
+
+template <int NT>
+__global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__ offsets, const u32* __restrict__ list,
+                                               u32* __restrict__ bits, u32* __restrict__ hdr) {
+    __shared__ u32 img[1024];
+    __shared__ __align__(16) int rec[NT][REC_W + 2];  // row = 20 words: int4-aligned
+    __shared__ u32 s_large;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = NT / 32;
+    const u32 b = blockIdx.x;
+    const u32 bx = b % p.nbx;
+    u32 rest = b / p.nbx;
+    const u32 by = rest % p.nby;
+    rest /= p.nby;
+    const u32 bz = rest % p.nbz;
+    const u32 m = rest / p.nbz;
+    const int X0 = bx << 5, Y0 = by << p.ty_log, Z0 = bz << p.tz_log;
+    const int rows = 1 << (p.ty_log + p.tz_log);
+    for (int i = tid; i < rows; i += NT) img[i] = 0;
+    if (tid == 0) s_large = 0;
+    const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
+    for (u32 base = beg; base < end; base += NT) {
+        __syncthreads();
+        const int n = min((u32)NT, end - base);
+        if (tid < n) setup_record(p, list[base + tid], X0, Y0, Z0, rec[tid]);
+        __syncthreads();
+        for (int i = warp; i < n; i += NW) {
+            const int* r = rec[i];
+            if (r[17] == KIND_FAST) {
+                raster_fast(r, img, lane, p.ty_log);
+            } else {
+                raster_large(p, (u32)r[0], (u32)r[16], X0, Y0, Z0, img, lane);
+                if (lane == 0) atomicAdd(&s_large, 1u);
+            }
+        }
+    }
+    __syncthreads();
+    const int TY = 1 << p.ty_log;
+    for (int i = tid; i < rows; i += NT) {
+        const int z = i >> p.ty_log, y = i & (TY - 1);
+        const int gy = Y0 + y, gz = Z0 + z;
+        if (gy < p.ny && gz < p.nz)
+            bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[img_idx(y, z, p.ty_log)];
+    }
+    if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
+}
+
+// ------------------------------------------------------------------------------------------
+// validation and probes
+// ------------------------------------------------------------------------------------------
+__global__ void k_validate(Params p, u32* hdr) {
+    i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    bool bad = false;
+    if (i < p.V) {
+        int x = p.verts[3 * i], y = p.verts[3 * i + 1], z = p.verts[3 * i + 2];
+        bad = bad || x < 0 || x > p.ex || y < 0 || y > p.ey || z < 0 || z > p.ez;
+    }
+    if (i < p.T) {
+        int4 id = p.tets[i];
+        bad = bad || id.x < 0 || id.x >= p.V || id.y < 0 || id.y >= p.V || id.z < 0 || id.z >= p.V || id.w < 0 || id.w >= p.V;
+    }
+    if (p.off && i <= p.batch) {
+        i64 o = p.off[i];
+        if (i == 0) bad = bad || (o != 0);
+        if (i == p.batch) bad = bad || (o != p.T);
+        if (i > 0) bad = bad || (o < p.off[i - 1]);
+    }
+    if (bad) hdr[H_BAD] = 1;
+}
+
+// dependent-free integer streams: 8 independent chains per thread
+template <int KIND>
+__global__ void __launch_bounds__(256) k_probe(int iters, u32* sink) {
+    u32 a0 = threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    u32 b = blockIdx.x * 2654435761u + 12345u, c = b ^ 0x9E3779B9u;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            if (KIND == 0) {  // LOP3 only: alu pipe
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a0) : "r"(b), "r"(c));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a1) : "r"(b), "r"(c));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a2) : "r"(b), "r"(c));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a3) : "r"(b), "r"(c));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a4) : "r"(b), "r"(c));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a5) : "r"(b), "r"(c));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a6) : "r"(b), "r"(c));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a7) : "r"(b), "r"(c));
+            } else if (KIND == 1) {  // IMAD only: fma pipe
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a0) : "r"(b), "r"(c));
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a1) : "r"(b), "r"(c));
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a2) : "r"(b), "r"(c));
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a3) : "r"(b), "r"(c));
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a4) : "r"(b), "r"(c));
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a5) : "r"(b), "r"(c));
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a6) : "r"(b), "r"(c));
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a7) : "r"(b), "r"(c));
+            } else {  // mixed: 4 LOP3 + 4 IMAD
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a0) : "r"(b), "r"(c));
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a1) : "r"(b), "r"(c));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a2) : "r"(b), "r"(c));
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a3) : "r"(b), "r"(c));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a4) : "r"(b), "r"(c));
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a5) : "r"(b), "r"(c));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a6) : "r"(b), "r"(c));
+                asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a7) : "r"(b), "r"(c));
+            }
+        }
+    }
+    u32 r = a0 ^ a1 ^ a2 ^ a3 ^ a4 ^ a5 ^ a6 ^ a7;
+    if (r == 0x12345678u) sink[0] = r;  // practically never: keeps the chains alive
+}
+
+// ------------------------------------------------------------------------------------------
+// host API
+// ------------------------------------------------------------------------------------------
+static int gcd_i(int a, int b) {
+    while (b) { int t = a % b; a = b; b = t; }
+    return a;
+}
+static int ilog2_exact(int v) {
+    for (int s = 0; s < 31; ++s) if ((1 << s) == v) return s;
+    return -1;
+}
+static int cuda_fail(vox_ctx* c, cudaError_t e, const char* where) {
+    snprintf(c->err, sizeof(c->err), "%s: %s", where, cudaGetErrorString(e));
+    return VOX_ECUDA;
+}
+#define CK(call)                                            \
+    do {                                                    \
+        cudaError_t e_ = (call);                            \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); \
+    } while (0)
+
+static void set_tile(Params& p, int ty, int tz) {
+    p.ty_log = ilog2_exact(ty);
+    p.tz_log = ilog2_exact(tz);
+    p.nbx = p.nx / 32;
+    p.nby = (p.ny + ty - 1) / ty;
+    p.nbz = (p.nz + tz - 1) / tz;
+    p.NB = (u32)((i64)p.batch * p.nbx * p.nby * p.nbz);
+}
+
+extern "C" int vox_create(vox_ctx** out, int nx, int ny, int nz, int ex, int ey, int ez, int batch) {
+    if (!out) return VOX_EINVAL;
+    *out = NULL;
+    if (nx <= 0 || ny <= 0 || nz <= 0 || batch < 1 || ex <= 0 || ey <= 0 || ez <= 0) return VOX_EINVAL;
+    if (nx % 32) return VOX_EINVAL;
+    if (ex % (2 * (i64)nx) || ey % (2 * (i64)ny) || ez % (2 * (i64)nz)) return VOX_EINVAL;
+    if (ex > (1 << 20) || ey > (1 << 20) || ez > (1 << 20)) return VOX_ERANGE;
+    if (nx > 32768 || ny > 32768 || nz > 32768) return VOX_ERANGE;
+    vox_ctx* c = (vox_ctx*)calloc(1, sizeof(vox_ctx));
+    if (!c) return VOX_EINVAL;
+    Params& p = c->p;
+    p.nx = nx; p.ny = ny; p.nz = nz; p.ex = ex; p.ey = ey; p.ez = ez; p.batch = batch;
+    p.hx = ex / nx; p.hy = ey / ny; p.hz = ez / nz;
+    p.g = gcd_i(gcd_i(p.hx, p.hy), p.hz);
+    p.g_shift = ilog2_exact(p.g);
+    p.sx = p.hx / p.g; p.sy = p.hy / p.g; p.sz = p.hz / p.g;
+    p.wpr = nx / 32;
+    // tile: 32^3 bricks for big grids; thinner tiles when there would be too few CTAs for 148 SMs
+    int ty = 32, tz = 32;
+    auto tiles = [&](int a, int b) { return (i64)batch * (nx / 32) * ((ny + a - 1) / a) * ((nz + b - 1) / b); };
+    while (tiles(ty, tz) < 1184 && (ty > 8 || tz > 8)) {  // 1184 = 8 CTAs x 148 SMs
+        if (tz >= ty && tz > 8) tz >>= 1; else ty >>= 1;
+    }
+    while (ty < 32 && (ny + ty - 1) / ty > 1024) ty <<= 1;
+    while (tz < 32 && (nz + tz - 1) / tz > 1024) tz <<= 1;
+    set_tile(p, ty, tz);
+    if (tiles(ty, tz) > 0xFFFFFFF0ll) { free(c); return VOX_ERANGE; }
+    c->pairs_planned = -1;
+    *out = c;
+    return VOX_OK;
+}
+
+extern "C" void vox_destroy(vox_ctx* ctx) { free(ctx); }
+
+extern "C" int vox_set_tile(vox_ctx* ctx, int ty, int tz) {
+    if (!ctx) return VOX_EINVAL;
+    if (ctx->have_tets) return VOX_ESTATE;
+    if (ilog2_exact(ty) < 2 || ty > 32 || ilog2_exact(tz) < 2 || tz > 32) return VOX_EINVAL;
+    if ((ctx->p.ny + ty - 1) / ty > 1024 || (ctx->p.nz + tz - 1) / tz > 1024) return VOX_ERANGE;
+    set_tile(ctx->p, ty, tz);
+    return VOX_OK;
+}
+
+extern "C" int vox_set_variant(vox_ctx* ctx, int variant) {
+    if (!ctx) return VOX_EINVAL;
+    ctx->variant = variant;
+    return VOX_OK;
+}
+
+extern "C" int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const int32_t* d_tets, int64_t T,
+                        const int64_t* d_tet_offsets) {
+    if (!ctx || V < 0 || T < 0) return VOX_EINVAL;
+    if (T > 0 && (!d_verts || !d_tets || V == 0)) return VOX_EINVAL;
+    if (ctx->p.batch > 1 && !d_tet_offsets) return VOX_EINVAL;
+    if (T > 0xFFFFFFF0ll || V > 0x7FFFFFFFll) return VOX_ERANGE;
+    if (((uintptr_t)d_tets & 15) != 0) return VOX_EINVAL;  // int4 loads
+    ctx->p.verts = d_verts;
+    ctx->p.tets = (const int4*)d_tets;
+    ctx->p.V = V;
+    ctx->p.T = T;
+    ctx->p.off = (ctx->p.batch > 1) ? (const i64*)d_tet_offsets : NULL;
+    ctx->have_tets = true;
+    ctx->pairs_planned = -1;
+    return VOX_OK;
+}
+
+extern "C" size_t vox_grid_words(const vox_ctx* ctx) {
+    if (!ctx) return 0;
+    const Params& p = ctx->p;
+    return (size_t)p.batch * p.nz * p.ny * p.wpr;
+}
+
+extern "C" size_t vox_workspace_fixed_bytes(const vox_ctx* ctx) {
+    if (!ctx) return 0;
+    return ws_layout(ctx->p).fixed_end;
+}
+
+extern "C" size_t vox_workspace_bytes(const vox_ctx* ctx) {
+    if (!ctx) return 0;
+    const Params& p = ctx->p;
+    i64 pairs = ctx->pairs_planned >= 0 ? ctx->pairs_planned : 4 * p.T + (i64)p.NB;
+    if (pairs < 1) pairs = 1;
+    return ws_layout(p).fixed_end + align256((size_t)pairs * 4);
+}
+
+static int enqueue_count_scan(vox_ctx* ctx, cudaStream_t st, char* ws) {
+    Params& p = ctx->p;
+    WsLayout L = ws_layout(p);
+    u32* hdr = (u32*)(ws + L.hdr);
+    u32* counts = (u32*)(ws + L.counts);
+    u32* cursor = (u32*)(ws + L.cursor);
+    uint2* range = (uint2*)(ws + L.range);
+    // header and counts are adjacent: one memset
+    CK(cudaMemsetAsync(ws + L.hdr, 0, L.cursor - L.hdr, st));
+    if (p.T > 0) {
+        unsigned blocks = (unsigned)((p.T + 255) / 256);
+        k1_count<<<blocks, 256, 0, st>>>(p, range, counts, hdr);
+    }
+    k2_scan<<<1, 1024, 0, st>>>(p.NB, counts, cursor, hdr);
+    CK(cudaGetLastError());
+    return VOX_OK;
+}
+
+extern "C" int vox_plan(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes, int64_t* pairs_out) {
+    if (!ctx || !d_workspace) return VOX_EINVAL;
+    if (!ctx->have_tets) return VOX_ESTATE;
+    WsLayout L = ws_layout(ctx->p);
+    if (ws_bytes < L.fixed_end) return VOX_EWORKSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = enqueue_count_scan(ctx, st, (char*)d_workspace);
+    if (rc) return rc;
+    u32 h[HDR_WORDS];
+    CK(cudaMemcpyAsync(h, (char*)d_workspace + L.hdr, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    i64 total = (i64)h[H_TOTAL] | ((i64)h[H_TOTAL_HI] << 32);
+    if (total > 0xFFFFFFF0ll) return VOX_ERANGE;
+    ctx->pairs_planned = total;
+    if (pairs_out) *pairs_out = total;
+    return VOX_OK;
+}
+
+extern "C" int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes, uint32_t* d_bits_out) {
+    if (!ctx || !d_workspace || !d_bits_out) return VOX_EINVAL;
+    if (!ctx->have_tets) return VOX_ESTATE;
+    Params& p = ctx->p;
+    WsLayout L = ws_layout(p);
+    if (ws_bytes < L.fixed_end + 4) return VOX_EWORKSPACE;
+    size_t cap = (ws_bytes - L.list) / 4;
+    p.cap = (u32)(cap > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : cap);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char* ws = (char*)d_workspace;
+    int rc = enqueue_count_scan(ctx, st, ws);
+    if (rc) return rc;
+    u32* hdr = (u32*)(ws + L.hdr);
+    u32* counts = (u32*)(ws + L.counts);
+    u32* cursor = (u32*)(ws + L.cursor);
+    uint2* range = (uint2*)(ws + L.range);
+    u32* list = (u32*)(ws + L.list);
+    if (p.T > 0) {
+        unsigned blocks = (unsigned)((p.T + 255) / 256);
+        k3_scatter<<<blocks, 256, 0, st>>>(p, range, cursor, list, hdr);
+    }
+    k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
+    CK(cudaGetLastError());
+    return VOX_OK;
+}
+
+extern "C" int vox_status(vox_ctx* ctx, void* cuda_stream, const void* d_workspace, int64_t stats_out[4]) {
+    if (!ctx || !d_workspace) return VOX_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    WsLayout L = ws_layout(ctx->p);
+    u32 h[HDR_WORDS];
+    CK(cudaMemcpyAsync(h, (const char*)d_workspace + L.hdr, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (stats_out) {
+        stats_out[0] = (i64)h[H_TOTAL] | ((i64)h[H_TOTAL_HI] << 32);
+        stats_out[1] = h[H_CULLED];
+        stats_out[2] = h[H_LARGE];
+        stats_out[3] = h[H_NONEMPTY];
+    }
+    return h[H_OVERFLOW] ? VOX_EWORKSPACE : VOX_OK;
+}
+
+extern "C" int vox_validate(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes) {
+    if (!ctx || !d_workspace) return VOX_EINVAL;
+    if (!ctx->have_tets) return VOX_ESTATE;
+    Params& p = ctx->p;
+    WsLayout L = ws_layout(p);
+    if (ws_bytes < L.fixed_end) return VOX_EWORKSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    u32* hdr = (u32*)((char*)d_workspace + L.hdr);
+    CK(cudaMemsetAsync(hdr, 0, HDR_WORDS * 4, st));
+    i64 n = p.V > p.T ? p.V : p.T;
+    if (n < p.batch + 1) n = p.batch + 1;
+    k_validate<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, hdr);
+    CK(cudaGetLastError());
+    u32 h[HDR_WORDS];
+    CK(cudaMemcpyAsync(h, hdr, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return h[H_BAD] ? VOX_EDATA : VOX_OK;
+}
+
+struct ArenaLayout {
+    size_t verts, tets, off, bits, ws, end;
+};
+static ArenaLayout arena_layout(const vox_ctx* ctx, i64 V, i64 T, size_t ws_bytes) {
+    ArenaLayout A;
+    size_t o = 0;
+    A.verts = o; o = align256(o + (size_t)(V > 0 ? V : 1) * 12);
+    A.tets = o;  o = align256(o + (size_t)(T > 0 ? T : 1) * 16);
+    A.off = o;   o = align256(o + ((size_t)ctx->p.batch + 1) * 8);
+    A.bits = o;  o = align256(o + vox_grid_words(ctx) * 4);
+    A.ws = o;    o = o + ws_bytes;
+    A.end = o;
+    return A;
+}
+
+extern "C" size_t vox_host_arena_bytes(const vox_ctx* ctx, int64_t V, int64_t T) {
+    if (!ctx) return 0;
+    vox_ctx tmp = *ctx;
+    tmp.p.T = T;
+    tmp.pairs_planned = -1;
+    return arena_layout(ctx, V, T, vox_workspace_bytes(&tmp)).end;
+}
+
+extern "C" int vox_run_host(vox_ctx* ctx, void* cuda_stream, const int32_t* h_verts, int64_t V, const int32_t* h_tets,
+                            int64_t T, const int64_t* h_tet_offsets, void* d_arena, size_t arena_bytes,
+                            uint32_t* h_bits_out) {
+    if (!ctx || !d_arena || !h_bits_out || V < 0 || T < 0) return VOX_EINVAL;
+    if (T > 0 && (!h_verts || !h_tets)) return VOX_EINVAL;
+    if (ctx->p.batch > 1 && !h_tet_offsets) return VOX_EINVAL;
+    ArenaLayout A = arena_layout(ctx, V, T, 0);
+    if (arena_bytes < A.ws + 4096) return VOX_EWORKSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char* a = (char*)d_arena;
+    if (V > 0) CK(cudaMemcpyAsync(a + A.verts, h_verts, (size_t)V * 12, cudaMemcpyHostToDevice, st));
+    if (T > 0) CK(cudaMemcpyAsync(a + A.tets, h_tets, (size_t)T * 16, cudaMemcpyHostToDevice, st));
+    if (ctx->p.batch > 1)
+        CK(cudaMemcpyAsync(a + A.off, h_tet_offsets, ((size_t)ctx->p.batch + 1) * 8, cudaMemcpyHostToDevice, st));
+    int rc = vox_tets(ctx, (const int32_t*)(a + A.verts), V, (const int32_t*)(a + A.tets), T, (const int64_t*)(a + A.off));
+    if (rc) return rc;
+    rc = vox_run(ctx, st, a + A.ws, arena_bytes - A.ws, (uint32_t*)(a + A.bits));
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(h_bits_out, a + A.bits, vox_grid_words(ctx) * 4, cudaMemcpyDeviceToHost, st));
+    return vox_status(ctx, st, a + A.ws, NULL);
+}
+
+extern "C" int vox_probe_int32(void* cuda_stream, int kind, int blocks, int iters, uint32_t* d_sink, double* ops_out) {
+    if (blocks <= 0 || iters <= 0 || !d_sink) return VOX_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (kind == 0) k_probe<0><<<blocks, 256, 0, st>>>(iters, d_sink);
+    else if (kind == 1) k_probe<1><<<blocks, 256, 0, st>>>(iters, d_sink);
+    else k_probe<2><<<blocks, 256, 0, st>>>(iters, d_sink);
+    if (cudaGetLastError() != cudaSuccess) return VOX_ECUDA;
+    if (ops_out) *ops_out = (double)blocks * 256.0 * (double)iters * 64.0;
+    return VOX_OK;
+}
+
+extern "C" const char* vox_strerror(int code) {
+    switch (code) {
+        case VOX_OK: return "ok";
+        case VOX_EINVAL: return "invalid argument";
+        case VOX_ERANGE: return "argument out of the supported range";
+        case VOX_EWORKSPACE: return "workspace too small";
+        case VOX_ECUDA: return "CUDA runtime error (see vox_last_error)";
+        case VOX_ESTATE: return "call order violated";
+        case VOX_EDATA: return "mesh data out of range";
+        default: return "unknown error";
+    }
+}
+
+extern "C" const char* vox_last_error(const vox_ctx* ctx) { return ctx ? ctx->err : ""; }

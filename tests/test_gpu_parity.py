@@ -1,0 +1,241 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, bit for bit.
+
+Integer work: the bar is bit-exact equality of the whole grid."""
+import numpy as np
+import pytest
+
+import meshgen
+import oracle
+from meshgen.kuhn import Mesh, kuhn_mesh
+
+pytestmark = pytest.mark.gpu
+E = 65536
+
+
+def gpu_voxelize(m, **kw):
+    import paper_2106_01326_b200 as pkg
+
+    off = m.tet_offsets if m.batch > 1 else None
+    return pkg.voxelize(m.verts, m.tets, m.grid, m.extent, tet_offsets=off, **kw)
+
+
+def cpu_voxelize(m):
+    return oracle.voxelize(m.verts, m.tets, m.grid, m.extent, tet_offsets=m.tet_offsets)
+
+
+def assert_same(got, exp, what=""):
+    if not np.array_equal(got, exp):
+        bad = np.argwhere(got != exp)
+        b = tuple(bad[0])
+        raise AssertionError(
+            f"{what}: {len(bad)} differing words; first at [m,z,y,xw]={b}: gpu={got[b]:#010x} oracle={exp[b]:#010x}; "
+            f"popcount gpu={int(np.unpackbits(got.view(np.uint8)).sum())} oracle={int(np.unpackbits(exp.view(np.uint8)).sum())}"
+        )
+
+
+def test_p1_single_tet():
+    m = meshgen.single_tet_mesh((0, 0, 0), (8192, 0, 0), (8192, 8192, 0), (8192, 8192, 8192))
+    got = gpu_voxelize(m)
+    assert_same(got, cpu_voxelize(m), "p1")
+    assert int(np.unpackbits(got.view(np.uint8)).sum()) == 20
+
+
+def _giant(grid=256, jitter=0.2, seed=1101):
+    m = meshgen.make_config("s1", seed)
+    if jitter == 0.0:
+        c = np.array([0, E // 2, E])
+        v, t = kuhn_mesh(c, c, c, 0.0, None)
+        m = Mesh("s1_nojit", v, t, (grid,) * 3, expect_all_ones=True)
+    return Mesh(m.name + f"_{grid}", m.verts, m.tets, (grid,) * 3, expect_all_ones=True)
+
+
+CASES = {
+    "cfg1": lambda: meshgen.make_config("cfg1"),
+    "cfg1_drop3": lambda: meshgen.carve_every_third(meshgen.make_config("cfg1")),
+    "cfg1_sphere": lambda: meshgen.carve_sphere(meshgen.make_config("cfg1")),
+    "cfg2": lambda: meshgen.make_config("cfg2"),
+    "cfg2_drop3": lambda: meshgen.carve_every_third(meshgen.make_config("cfg2")),
+    "cfg3_small": lambda: meshgen.make_config("cfg3_small"),
+    "cfg4_small": lambda: meshgen.make_config("cfg4_small"),
+    "cfg4_small_drop3": lambda: meshgen.carve_every_third(meshgen.make_config("cfg4_small")),
+    "giant256": lambda: _giant(256),
+    "giant256_nojit": lambda: _giant(256, 0.0),
+    "giant256_drop3": lambda: meshgen.carve_every_third(_giant(256)),
+    "giant128_sphere": lambda: meshgen.carve_sphere(_giant(128), 0.45),
+}
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_parity_small_configs(name):
+    m = CASES[name]()
+    exp = cpu_voxelize(m)
+    got = gpu_voxelize(m)
+    assert_same(got, exp, name)
+    if m.expect_all_ones:
+        assert np.all(got == np.uint32(0xFFFFFFFF))
+
+
+@pytest.mark.parametrize("tile", [(32, 32), (8, 8), (16, 4), (4, 32), (32, 4)])
+@pytest.mark.parametrize("name", ["cfg2", "cfg4_small_drop3", "giant128_sphere"])
+def test_parity_is_tile_independent(name, tile):
+    m = CASES[name]()
+    assert_same(gpu_voxelize(m, tile=tile), cpu_voxelize(m), f"{name} tile={tile}")
+
+
+def test_estimated_workspace_path():
+    m = CASES["cfg2"]()
+    assert_same(gpu_voxelize(m, exact_plan=False), cpu_voxelize(m), "cfg2 without vox_plan")
+
+
+def test_host_buffer_entry_point():
+    import paper_2106_01326_b200 as pkg
+
+    for name in ["cfg2", "cfg3_small"]:
+        m = CASES[name]()
+        off = m.tet_offsets if m.batch > 1 else None
+        got = pkg.voxelize_host(m.verts, m.tets, m.grid, m.extent, tet_offsets=off)
+        assert_same(got, cpu_voxelize(m), name + " via vox_run_host")
+
+
+# ------------------------------------------------------------------ edge cases
+def test_empty_mesh_gives_zero_grid():
+    m = Mesh("empty", np.zeros((4, 3), np.int32), np.zeros((0, 4), np.int32), (64, 32, 32))
+    got = gpu_voxelize(m)
+    assert got.shape == (1, 32, 32, 2) and not got.any()
+
+
+def test_all_tets_culled():
+    # degenerate (coplanar, repeated vertex) and sub-voxel slivers between sample planes
+    v = np.array([[0, 0, 1024], [E, 0, 1024], [0, E, 1024], [E, E, 1024],
+                  [10, 10, 10], [500, 10, 10], [10, 500, 10], [10, 10, 500]], dtype=np.int32)
+    t = np.array([[0, 1, 2, 3], [0, 1, 2, 2], [1, 1, 1, 1], [4, 5, 6, 7]], dtype=np.int32)
+    m = Mesh("culled", v, t, (32, 32, 32))
+    got = gpu_voxelize(m)
+    assert not got.any() and not cpu_voxelize(m).any()
+    import paper_2106_01326_b200 as pkg
+
+    assert pkg.voxelize.last_status["culled"] == 4 and pkg.voxelize.last_status["pairs"] == 0
+
+
+def test_stale_output_is_overwritten():
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    m = CASES["cfg1_sphere"]()
+    vz = pkg.Voxelizer(m.grid)
+    vz.set_tets(torch.from_numpy(m.verts).cuda(), torch.from_numpy(m.tets).cuda())
+    out = torch.full((1, 32, 32, 1), -1, dtype=torch.int32, device="cuda")
+    vz.plan()
+    vz.run(out)
+    vz.run(out)  # twice into the same buffers: no stale state in the workspace either
+    vz.status()
+    assert_same(out.cpu().numpy().view(np.uint32), cpu_voxelize(m), "rerun")
+    vz.close()
+
+
+@pytest.mark.parametrize(
+    "grid,extent",
+    [((32, 24, 40), (32 * 6, 24 * 10, 40 * 14)),     # pitches 6,10,14: gcd 2
+     ((64, 20, 12), (64 * 6, 20 * 12, 12 * 18)),     # pitches 6,12,18: gcd 6 (not a power of two)
+     ((32, 40, 24), (32 * 2048, 40 * 512, 24 * 4096)),
+     ((96, 33, 7), (96 * 4, 33 * 4, 7 * 4))],
+)
+def test_ragged_anisotropic_grids(grid, extent):
+    rng = np.random.default_rng(sum(grid))
+    cs = [np.rint(np.linspace(0, extent[k], 4 + k)).astype(np.int64) for k in range(3)]
+    v, t = kuhn_mesh(cs[0], cs[1], cs[2], 0.2, rng)
+    # move boundary vertices too (kept inside the box), then carve
+    v = np.clip(v + rng.integers(-2, 3, v.shape), 0, np.array(extent)).astype(np.int32)
+    t = t[rng.random(len(t)) < 0.7]
+    m = Mesh("ragged", v, t, grid, extent)
+    exp = cpu_voxelize(m)
+    assert exp.any() and not np.all(exp == np.uint32(0xFFFFFFFF))
+    for tile in [None, (4, 4), (16, 8)]:
+        assert_same(gpu_voxelize(m, tile=tile), exp, f"ragged {grid} tile={tile}")
+
+
+def test_max_extent_forces_the_int64_large_path():
+    # extent 2^20: plane coefficients exceed int32 on every tile
+    Emax = 1 << 20
+    rng = np.random.default_rng(5)
+    c = np.rint(np.linspace(0, Emax, 4)).astype(np.int64)
+    v, t = kuhn_mesh(c, c, c, 0.2, rng)
+    t = t[rng.random(len(t)) < 0.6]
+    m = Mesh("emax", v, t, (64, 64, 64), (Emax,) * 3)
+    got = gpu_voxelize(m)
+    assert_same(got, cpu_voxelize(m), "extent 2^20")
+    import paper_2106_01326_b200 as pkg
+
+    assert pkg.voxelize.last_status["large_pairs"] > 0
+
+
+def test_random_soup_with_overlaps_and_inverted_tets():
+    # not a conforming mesh: random tets of all sizes, both orientations, overlapping
+    rng = np.random.default_rng(77)
+    v = rng.integers(0, E + 1, (400, 3)).astype(np.int32)
+    t = np.array([rng.choice(400, 4, replace=False) for _ in range(300)], dtype=np.int32)
+    small = (v[:200] // 16 + 30000).astype(np.int32)  # a cluster of small tets
+    v[:200] = small
+    m = Mesh("soup", v, t, (64, 64, 64))
+    assert_same(gpu_voxelize(m), cpu_voxelize(m), "soup")
+
+
+def test_vertices_on_sample_points_and_faces():
+    # coordinates on multiples of h/2: samples exactly on faces, edges and vertices (inclusive test)
+    rng = np.random.default_rng(61)
+    h = 2048
+    pts = (rng.integers(0, 65, (60, 3)) * (h // 2)).astype(np.int32)
+    t = np.array([rng.choice(60, 4, replace=False) for _ in range(120)], dtype=np.int32)
+    m = Mesh("onfaces", pts, t, (32, 32, 32))
+    assert_same(gpu_voxelize(m), cpu_voxelize(m), "on-faces")
+    h = 512
+    pts = (rng.integers(40, 90, (80, 3)) * (h // 2)).astype(np.int32)  # small tets: int32 fast path
+    t = np.array([rng.choice(80, 4, replace=False) for _ in range(200)], dtype=np.int32)
+    m = Mesh("onfaces_small", pts, t, (128, 128, 128))
+    assert_same(gpu_voxelize(m), cpu_voxelize(m), "on-faces small")
+
+
+def test_workspace_overflow_is_reported():
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    m = CASES["cfg2"]()
+    vz = pkg.Voxelizer(m.grid)
+    vz.set_tets(torch.from_numpy(m.verts).cuda(), torch.from_numpy(m.tets).cuda())
+    vz.alloc_workspace(vz.workspace_fixed_bytes + 4096)  # room for 1024 pairs only
+    vz.run()
+    with pytest.raises(pkg.VoxError) as ei:
+        vz.status()
+    assert ei.value.code == -3
+    pairs = vz.plan()
+    assert pairs > 1024
+    vz.run()
+    assert vz.status()["pairs"] == pairs
+    vz.close()
+
+
+def test_validate_flags_bad_data():
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    m = CASES["cfg1"]()
+    vz = pkg.Voxelizer(m.grid)
+    v = torch.from_numpy(m.verts).cuda()
+    t = torch.from_numpy(m.tets).cuda()
+    vz.set_tets(v, t)
+    vz.validate()
+    t2 = t.clone()
+    t2[5, 2] = m.V
+    vz.set_tets(v, t2)
+    with pytest.raises(pkg.VoxError) as ei:
+        vz.validate()
+    assert ei.value.code == -6
+    v2 = v.clone()
+    v2[3, 1] = E + 1
+    vz.set_tets(v2, t)
+    with pytest.raises(pkg.VoxError):
+        vz.validate()
+    vz.close()
