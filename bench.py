@@ -1,0 +1,417 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the tet-mesh -> solid-bit-grid hot path on B200.
+
+One "step" = one vox_run (K1 count, K2 scan, K3 scatter, K4 brick voxelizer incl. the
+large-tet path; every word of the grid written) over one synthetic mesh of the workload.
+Default workload = BASELINE.json configs[3] ("cfg4": ~4.8M tets, 1024^3 grid), the
+configuration the metric is quoted on.  DESIGN.md "Measurement" defines every number.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--impl reference]
+
+Prints ONE JSON line (rank 0).  With --gpus N > 1 it expects to be launched by
+torch.distributed.run (one rank per GPU): every rank voxelizes its own replica of the
+workload (seed + rank), no data-path collective ("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Gvoxel-samples/s"
+UNIT = "Gvoxel-samples/s"
+# INT32 model frozen in DESIGN.md "Roofline": ops the method itself must execute
+OPS_PER_SAMPLE = 11.0
+OPS_PER_PAIR = 150.0
+# alu-pipe peak: 148 SMs x 64 INT32 lanes/clk x clocks.max.sm (B300_MICROARCH "Pipe rates":
+# IADD3/LOP3/SHF rt_SMSP = 2 -> 16 lanes/clk/SMSP -> 64/SM); DESIGN.md "Roofline"
+ALU_LANES_PER_SM = 64
+
+
+def _args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="cfg4")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--tile", type=int, nargs=2, default=None)
+    return ap.parse_args()
+
+
+def candidate_samples(m):
+    """Sum over tets of |closed bbox(t) /\\ voxel-centre lattice| (PAPER.md:98's unit of work).
+
+    Pure bookkeeping on the input arrays (min/max, floor division); culled slivers count 0,
+    degenerate tets count their bbox like any other (the GPU has to look at them too)."""
+    import numpy as np
+
+    total = 0
+    step = 1 << 20
+    for s in range(0, m.T, step):
+        v = m.verts[m.tets[s : s + step]].astype(np.int64)  # [t][4][3]
+        lo, hi = v.min(axis=1), v.max(axis=1)
+        cnt = np.ones(len(v), dtype=np.int64)
+        for a in range(3):
+            h = m.extent[a] // m.grid[a]
+            i0 = np.maximum(-((h - 2 * lo[:, a]) // (2 * h)), 0)
+            i1 = np.minimum((2 * hi[:, a] - h) // (2 * h), m.grid[a] - 1)
+            cnt *= np.maximum(i1 - i0 + 1, 0)
+        total += int(cnt.sum())
+    return total
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.004):
+        self.index, self.period = index, period
+        self.sm, self.reasons, self.power = [], set(), []
+        self.sm_max = None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception as e:  # pragma: no cover
+            self.nv = None
+            self.err = repr(e)
+
+    _NAMES = {
+        0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x10: "sync_boost",
+        0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
+        0x100: "display_clock_setting",
+    }
+
+    def _loop(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h) if hasattr(
+                    nv, "nvmlDeviceGetCurrentClocksEventReasons") else nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in self._NAMES.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:  # pragma: no cover
+                pass
+            time.sleep(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if self.nv is None or not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": [], "note": "nvml unavailable"}
+        return {
+            "sm_mhz": statistics.median(self.sm), "sm_min_mhz": min(self.sm), "sm_max_mhz": self.sm_max,
+            "reasons": sorted(self.reasons), "samples": len(self.sm),
+            "power_w_max": max(self.power) if self.power else None,
+        }
+
+
+# ------------------------------------------------------------------------------------------
+# the oracle timed on the host cores (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------
+def time_oracle(m, target_s=12.0, repeats=1):
+    """Times oracle.voxelize as it stands on a bounded sample: every `stride`-th tet of the
+    workload (the oracle's own tet_stride argument).  Returns (samples/s, info dict)."""
+    import oracle
+
+    cores = oracle.num_threads()
+    # two-point calibration (the fixed cost of zero-filling the grid cancels), then aim for target_s
+    def once(stride):
+        t0 = time.perf_counter()
+        _, s = oracle.voxelize(m.verts, m.tets, m.grid, m.extent, tet_offsets=m.tet_offsets,
+                               tet_stride=stride, return_samples=True)
+        return s, time.perf_counter() - t0
+
+    sa, ta = once(max(1, m.T // 4096))
+    sb, tb = once(max(1, m.T // 65536))
+    rate0 = (sa - sb) / max(ta - tb, 1e-4) if sa > sb else max(sa, 1) / max(ta, 1e-4)
+    total = candidate_samples(m)
+    want = rate0 * target_s
+    stride = max(1, int(total / max(want, 1.0)))
+    best = None
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        _, s = oracle.voxelize(m.verts, m.tets, m.grid, m.extent, tet_offsets=m.tet_offsets,
+                               tet_stride=stride, return_samples=True)
+        dt = time.perf_counter() - t0
+        if best is None or dt < best[0]:
+            best = (dt, s)
+    dt, s = best
+    info = {
+        "kind": "oracle", "cores": cores,
+        "sample": f"every {stride}th tet of {m.name} ({-(-m.T // stride)} of {m.T} tets, {s} candidate samples, "
+                  f"{dt:.2f} s wall incl. zero-filling the grid)",
+        "seconds": dt, "samples": s, "stride": stride,
+    }
+    return s / dt, info
+
+
+def run_reference(args):
+    """--impl reference: the oracle (unmodified) on the host cores, same metric/config."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import meshgen
+    import oracle
+
+    m = meshgen.make_config(args.workload)
+    total = candidate_samples(m)
+    # size a step so that warmup+steps finish in ~2-3 minutes
+    per_step_s = max(1.0, min(15.0, 150.0 / max(1, args.steps + args.warmup)))
+    rate, info = time_oracle(m, target_s=per_step_s)
+    stride = info["stride"]
+    times, samples = [], 0
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        _, s = oracle.voxelize(m.verts, m.tets, m.grid, m.extent, tet_offsets=m.tet_offsets,
+                               tet_stride=stride, return_samples=True)
+        dt = time.perf_counter() - t0
+        if i >= args.warmup:
+            times.append(dt)
+            samples += s
+    tsum = sum(times)
+    value = samples / tsum / 1e9
+    info["sample"] = (f"each step = every {stride}th tet of {m.name} ({-(-m.T // stride)} of {m.T} tets, "
+                      f"{samples // max(1, args.steps)} candidate samples)")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tsum / max(1, args.steps),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
+        "data": "synthetic",
+        "config": {"workload": m.name, "tets": m.T, "verts": m.V, "grid": list(m.grid),
+                   "candidate_samples_full": total, "bounded_sample_stride": stride},
+        "mtets_per_s": (-(-m.T // stride)) * args.steps / tsum / 1e6,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
+                         "sample": info["sample"]},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------
+# the CUDA path
+# ------------------------------------------------------------------------------------------
+def run_b200(args):
+    import numpy as np
+    import torch
+
+    import meshgen
+    import paper_2106_01326_b200 as pkg
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    pkg.load_library()  # fail loudly if libvox.so is missing
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    # replicas: rank r voxelizes its own mesh of the same recipe (default seed + r)
+    base = meshgen.make_config(args.workload, None) if rank == 0 else None
+    if rank == 0:
+        m = base
+    else:
+        from meshgen.kuhn import _CONFIGS
+
+        m = meshgen.make_config(args.workload, _CONFIGS[args.workload][1] + rank)
+    samples = candidate_samples(m)
+
+    stream = torch.cuda.Stream()
+    off_np = m.tet_offsets if m.batch > 1 else None
+    with torch.cuda.stream(stream):
+        d_verts = torch.from_numpy(m.verts).cuda()
+        d_tets = torch.from_numpy(m.tets).cuda()
+        d_off = torch.from_numpy(off_np).cuda() if off_np is not None else None
+        vz = pkg.Voxelizer(m.grid, m.extent, m.batch, tile=args.tile, variant=args.variant)
+        vz.set_tets(d_verts, d_tets, d_off)
+        pairs = vz.plan(stream)  # exact workspace sizing: outside the timed region (one sync)
+        vz.alloc_workspace()
+        nx, ny, nz = m.grid
+        out = torch.empty((m.batch, nz, ny, nx // 32), dtype=torch.int32, device="cuda")
+        vz.timing_enable(args.steps)
+
+        def barrier():
+            if dist is not None:
+                dist.barrier()
+
+        for _ in range(args.warmup):
+            vz.run(out, stream)
+        stream.synchronize()
+        st = vz.status(stream)
+        vz.timing_enable(args.steps)  # restart run numbering at 0 for the timed steps
+        barrier()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with ClockSampler(local_rank) as clk:
+            e0.record(stream)
+            for _ in range(args.steps):
+                vz.run(out, stream)
+            e1.record(stream)
+            barrier()
+            torch.cuda.synchronize()
+        ms_total = e0.elapsed_time(e1)
+        per = [vz.timing_read(i) for i in range(args.steps)]
+        vz.timing_enable(0)
+        popcount = None
+        if rank == 0:
+            popcount = int(np.unpackbits(out.cpu().numpy().view(np.uint8)).sum())
+
+        # max over ranks of the device time; sum over ranks of the work
+        tmax, ssum, tsum = ms_total, float(samples), float(m.T)
+        if dist is not None:
+            t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            w = torch.tensor([float(samples), float(m.T)], dtype=torch.float64, device="cuda")
+            dist.all_reduce(w, op=dist.ReduceOp.SUM)
+            tmax, ssum, tsum = float(t[0]), float(w[0]), float(w[1])
+        sec = tmax * 1e-3
+        value = ssum * args.steps / sec / 1e9
+
+        # ---- e2e: HOST buffers through vox_run_host (H2D of the mesh, run, D2H of the grid)
+        e2e = None
+        if not args.no_e2e:
+            hv = torch.from_numpy(m.verts).pin_memory()
+            ht = torch.from_numpy(m.tets).pin_memory()
+            ho = torch.from_numpy(off_np).pin_memory() if off_np is not None else None
+            hout = torch.empty((m.batch, nz, ny, nx // 32), dtype=torch.int32).pin_memory()
+            vz2 = pkg.Voxelizer(m.grid, m.extent, m.batch, tile=args.tile, variant=args.variant)
+            need = vz2.host_arena_bytes(m.V, m.T)
+            arena = torch.empty(need, dtype=torch.uint8, device="cuda")
+            for _ in range(2):
+                vz2.run_host(hv, ht, hout, arena, ho, stream)
+            barrier()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            f0.record(stream)
+            for _ in range(args.e2e_steps):
+                vz2.run_host(hv, ht, hout, arena, ho, stream)  # synchronises each step
+            f1.record(stream)
+            torch.cuda.synchronize()
+            wall = time.perf_counter() - t0
+            e2e_ms = max(f0.elapsed_time(f1), wall * 1e3)
+            if dist is not None:
+                t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                e2e_ms = float(t[0])
+            h2d = hv.numel() * 4 + ht.numel() * 4 + (ho.numel() * 8 if ho is not None else 0)
+            d2h = hout.numel() * 4 + 256  # grid + the status header
+            e2e = {"value": ssum * args.e2e_steps / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
+                   "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.e2e_steps,
+                   "steps": args.e2e_steps,
+                   "same_result": bool(rank != 0 or torch.equal(hout, out.cpu()))}
+            vz2.close()
+            del arena
+
+        if rank != 0:
+            vz.close()
+            if dist is not None:
+                dist.destroy_process_group()
+            return
+
+        # ---- roofline of the dominant kernel (K4), from the live per-kernel events
+        k4 = statistics.mean(p["k4"] for p in per)
+        shares = {k: statistics.mean(p[k] for p in per) for k in ("k1", "k2", "k3", "k4", "total")}
+        sm_max = clk.sm_max or 1965
+        peak_alu = 148 * ALU_LANES_PER_SM * sm_max * 1e6 / 1e12  # Tops/s
+        ops = OPS_PER_SAMPLE * samples + OPS_PER_PAIR * pairs
+        achieved = ops / (k4 * 1e-3) / 1e12
+        try:
+            probe = {k: pkg.probe_int32(kind=i) / 1e12 for i, k in enumerate(("alu_lop3", "fma_imad", "mixed"))}
+        except Exception as e:  # pragma: no cover
+            probe = {"error": repr(e)}
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        hbm_peak = peaks.get("hbm_gbs", 6650.0)
+        min_bytes = 16.0 * m.T + 12.0 * m.V + 4.0 * vz.grid_words
+        k4_bytes = 4.0 * vz.grid_words + pairs * (4.0 + 16.0 + 48.0)  # grid + per pair: id, tet, 4 verts
+        roofline = {
+            "bound": "alu", "kernel": "k4_brick", "achieved": achieved, "peak": peak_alu, "unit": "Tops/s (INT32)",
+            "frac": achieved / peak_alu, "traffic": None,
+            "model": f"{OPS_PER_SAMPLE:g} ops/candidate sample + {OPS_PER_PAIR:g} ops/(tet,tile) pair",
+            "ops_per_launch": ops, "kernel_ms": k4,
+            "peak_source": "derived: 148 SMs x 64 alu-pipe lanes x clocks.max.sm (DESIGN.md Roofline)",
+            "peak_probe_tops": probe,
+            "hbm": {"achieved_gbs": k4_bytes / (k4 * 1e-3) / 1e9, "peak_gbs": hbm_peak,
+                    "frac": k4_bytes / (k4 * 1e-3) / 1e9 / hbm_peak,
+                    "peak_source": "MEASURED_PEAKS.json (measured)" if peaks else "fallback",
+                    "k4_bytes_per_launch": k4_bytes, "whole_path_min_bytes": min_bytes,
+                    "whole_path_frac": min_bytes / (shares["total"] * 1e-3) / 1e9 / hbm_peak},
+        }
+
+        cpu = None
+        if not args.no_cpu_baseline:
+            rate, info = time_oracle(base, target_s=12.0)
+            cpu = {"value": rate / 1e9, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
+                   "sample": info["sample"]}
+
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": tmax / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int32/int64 (exact integer)", "data": "synthetic",
+            "config": {"workload": m.name, "tets": m.T, "verts": m.V, "grid": list(m.grid), "batch": m.batch,
+                       "candidate_samples": samples, "pairs": pairs, "tile": [32, 1 << 0, 1 << 0],
+                       "l2": "no flush: one step streams tets+verts+pair list+grid = "
+                             f"{(16 * m.T + 12 * m.V + 8 * m.T + 4 * pairs * 2 + 4 * vz.grid_words) / 1e6:.0f} MB > 126 MB L2",
+                       "multi_gpu": "replicas only (seed + rank), no collective"},
+            "mtets_per_s": tsum * args.steps / sec / 1e6,
+            "gvoxels_per_s": world * m.batch * nx * ny * nz * args.steps / sec / 1e9,
+            "kernel_ms": shares, "status": st, "popcount": popcount,
+            "gpu_launches": args.steps * 4 + (args.e2e_steps * 4 if e2e else 0),
+            "clocks": clk.summary(), "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+        }
+        line["config"].pop("tile")
+        print(json.dumps(line), flush=True)
+        vz.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = _args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

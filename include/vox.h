@@ -119,6 +119,17 @@ int vox_run_host(vox_ctx* ctx, void* cuda_stream, const int32_t* h_verts, int64_
                  const int32_t* h_tets, int64_t T, const int64_t* h_tet_offsets,
                  void* d_arena, size_t arena_bytes, uint32_t* h_bits_out);
 
+/* Benchmark instrumentation (off by default).  vox_timing_enable(ctx, slots > 0)
+ * creates a ring of CUDA events (a host-side allocation: call it outside any timed
+ * region); every later vox_run then records an event on its stream before K1's
+ * memset and after each of K1, K2, K3, K4 (no synchronisation).  Runs are numbered
+ * 0,1,2,... from the enable call.  vox_timing_read(ctx, run, ms) returns the
+ * durations {K1 incl. memset, K2, K3, K4, whole run} in milliseconds of a run that
+ * has COMPLETED (the caller synchronises) and is still in the ring, else VOX_ESTATE.
+ * slots == 0 disables and frees. */
+int vox_timing_enable(vox_ctx* ctx, int slots);
+int vox_timing_read(vox_ctx* ctx, int run, float ms_out[5]);
+
 /* Roofline probe (not on the hot path): enqueue a dependent-free integer kernel
  * on `cuda_stream`.  kind 0 = IADD3/LOP3 stream (alu pipe), 1 = IMAD stream
  * (fma pipe), 2 = mixed.  *ops_out = thread-level INT32 ops it executes. */

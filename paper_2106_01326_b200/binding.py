@@ -12,8 +12,8 @@ _lib = None
 EXPORTS = [
     "vox_create", "vox_destroy", "vox_set_tile", "vox_set_variant", "vox_tets", "vox_grid_words",
     "vox_workspace_bytes", "vox_workspace_fixed_bytes", "vox_plan", "vox_run", "vox_status",
-    "vox_validate", "vox_host_arena_bytes", "vox_run_host", "vox_probe_int32", "vox_strerror",
-    "vox_last_error",
+    "vox_validate", "vox_host_arena_bytes", "vox_run_host", "vox_timing_enable", "vox_timing_read",
+    "vox_probe_int32", "vox_strerror", "vox_last_error",
 ]
 
 
@@ -54,6 +54,8 @@ def load_library():
         "vox_validate": (i32, [vp, vp, vp, sz]),
         "vox_host_arena_bytes": (sz, [vp, i64, i64]),
         "vox_run_host": (i32, [vp, vp, vp, i64, vp, i64, vp, vp, sz, vp]),
+        "vox_timing_enable": (i32, [vp, i32]),
+        "vox_timing_read": (i32, [vp, i32, ctypes.POINTER(ctypes.c_float)]),
         "vox_probe_int32": (i32, [vp, i32, i32, i32, vp, ctypes.POINTER(ctypes.c_double)]),
         "vox_strerror": (ctypes.c_char_p, [i32]),
         "vox_last_error": (ctypes.c_char_p, [vp]),
@@ -210,6 +212,16 @@ class Voxelizer:
                                    self._ws.numel()),
             "vox_validate",
         )
+
+    # -- per-kernel device timing (benchmark instrumentation) -----------------------------
+    def timing_enable(self, slots):
+        self._ck(self._lib.vox_timing_enable(self._ctx, int(slots)), "vox_timing_enable")
+
+    def timing_read(self, run):
+        """dict of milliseconds for a completed run (numbered from timing_enable)."""
+        ms = (ctypes.c_float * 5)()
+        self._ck(self._lib.vox_timing_read(self._ctx, int(run), ms), "vox_timing_read")
+        return dict(k1=ms[0], k2=ms[1], k3=ms[2], k4=ms[3], total=ms[4])
 
     # -- host-buffer end-to-end path (vox_run_host) ---------------------------------------
     def host_arena_bytes(self, V, T):

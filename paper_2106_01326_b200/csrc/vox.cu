@@ -49,8 +49,12 @@ struct vox_ctx {
     bool have_tets;
     i64 pairs_planned;  // -1 = unknown
     int variant;
+    int tm_slots;        // per-kernel timing ring (0 = off)
+    int tm_next;
+    cudaEvent_t* tm_ev;  // [tm_slots][TM_EV]
     char err[256];
 };
+enum { TM_EV = 5 };  // before memset/K1, after K1, after K2, after K3, after K4
 
 enum { HDR_WORDS = 64 };
 // header words
@@ -607,7 +611,41 @@ extern "C" int vox_create(vox_ctx** out, int nx, int ny, int nz, int ex, int ey,
     return VOX_OK;
 }
 
-extern "C" void vox_destroy(vox_ctx* ctx) { free(ctx); }
+static void timing_free(vox_ctx* ctx) {
+    if (ctx->tm_ev) {
+        for (int i = 0; i < ctx->tm_slots * TM_EV; ++i) cudaEventDestroy(ctx->tm_ev[i]);
+        free(ctx->tm_ev);
+    }
+    ctx->tm_ev = NULL;
+    ctx->tm_slots = 0;
+    ctx->tm_next = 0;
+}
+
+extern "C" void vox_destroy(vox_ctx* ctx) {
+    if (!ctx) return;
+    timing_free(ctx);
+    free(ctx);
+}
+
+extern "C" int vox_timing_enable(vox_ctx* ctx, int slots) {
+    if (!ctx || slots < 0 || slots > 65536) return VOX_EINVAL;
+    timing_free(ctx);
+    if (slots == 0) return VOX_OK;
+    ctx->tm_ev = (cudaEvent_t*)calloc((size_t)slots * TM_EV, sizeof(cudaEvent_t));
+    if (!ctx->tm_ev) return VOX_EINVAL;
+    ctx->tm_slots = slots;
+    for (int i = 0; i < slots * TM_EV; ++i) CK(cudaEventCreate(&ctx->tm_ev[i]));
+    return VOX_OK;
+}
+
+extern "C" int vox_timing_read(vox_ctx* ctx, int run, float ms_out[5]) {
+    if (!ctx || !ms_out || run < 0) return VOX_EINVAL;
+    if (!ctx->tm_ev || run >= ctx->tm_next || run < ctx->tm_next - ctx->tm_slots) return VOX_ESTATE;
+    cudaEvent_t* e = ctx->tm_ev + (size_t)(run % ctx->tm_slots) * TM_EV;
+    for (int k = 0; k < 4; ++k) CK(cudaEventElapsedTime(ms_out + k, e[k], e[k + 1]));
+    CK(cudaEventElapsedTime(ms_out + 4, e[0], e[4]));
+    return VOX_OK;
+}
 
 extern "C" int vox_set_tile(vox_ctx* ctx, int ty, int tz) {
     if (!ctx) return VOX_EINVAL;
@@ -660,21 +698,24 @@ extern "C" size_t vox_workspace_bytes(const vox_ctx* ctx) {
     return ws_layout(p).fixed_end + align256((size_t)pairs * 4);
 }
 
-static int enqueue_count_scan(vox_ctx* ctx, cudaStream_t st, char* ws) {
+static int enqueue_count_scan(vox_ctx* ctx, cudaStream_t st, char* ws, cudaEvent_t* ev) {
     Params& p = ctx->p;
     WsLayout L = ws_layout(p);
     u32* hdr = (u32*)(ws + L.hdr);
     u32* counts = (u32*)(ws + L.counts);
     u32* cursor = (u32*)(ws + L.cursor);
     uint2* range = (uint2*)(ws + L.range);
+    if (ev) CK(cudaEventRecord(ev[0], st));
     // header and counts are adjacent: one memset
     CK(cudaMemsetAsync(ws + L.hdr, 0, L.cursor - L.hdr, st));
     if (p.T > 0) {
         unsigned blocks = (unsigned)((p.T + 255) / 256);
         k1_count<<<blocks, 256, 0, st>>>(p, range, counts, hdr);
     }
+    if (ev) CK(cudaEventRecord(ev[1], st));
     k2_scan<<<1, 1024, 0, st>>>(p.NB, counts, cursor, hdr);
     CK(cudaGetLastError());
+    if (ev) CK(cudaEventRecord(ev[2], st));
     return VOX_OK;
 }
 
@@ -684,7 +725,7 @@ extern "C" int vox_plan(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size
     WsLayout L = ws_layout(ctx->p);
     if (ws_bytes < L.fixed_end) return VOX_EWORKSPACE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int rc = enqueue_count_scan(ctx, st, (char*)d_workspace);
+    int rc = enqueue_count_scan(ctx, st, (char*)d_workspace, NULL);
     if (rc) return rc;
     u32 h[HDR_WORDS];
     CK(cudaMemcpyAsync(h, (char*)d_workspace + L.hdr, sizeof(h), cudaMemcpyDeviceToHost, st));
@@ -706,7 +747,8 @@ extern "C" int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_
     p.cap = (u32)(cap > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : cap);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char* ws = (char*)d_workspace;
-    int rc = enqueue_count_scan(ctx, st, ws);
+    cudaEvent_t* ev = ctx->tm_ev ? ctx->tm_ev + (size_t)(ctx->tm_next % ctx->tm_slots) * TM_EV : NULL;
+    int rc = enqueue_count_scan(ctx, st, ws, ev);
     if (rc) return rc;
     u32* hdr = (u32*)(ws + L.hdr);
     u32* counts = (u32*)(ws + L.counts);
@@ -717,8 +759,13 @@ extern "C" int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_
         unsigned blocks = (unsigned)((p.T + 255) / 256);
         k3_scatter<<<blocks, 256, 0, st>>>(p, range, cursor, list, hdr);
     }
+    if (ev) CK(cudaEventRecord(ev[3], st));
     k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
     CK(cudaGetLastError());
+    if (ev) {
+        CK(cudaEventRecord(ev[4], st));
+        ctx->tm_next++;
+    }
     return VOX_OK;
 }
 
