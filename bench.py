@@ -379,7 +379,7 @@ def run_b200(args):
 
         cpu = None
         if not args.no_cpu_baseline:
-            rate, info = time_oracle(base, target_s=12.0)
+            rate, info = time_oracle(base, target_s=12.0, repeats=3)
             cpu = {"value": rate / 1e9, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
                    "sample": info["sample"]}
 
