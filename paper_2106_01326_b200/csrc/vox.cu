@@ -485,6 +485,165 @@ __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__
 }
 
 // ------------------------------------------------------------------------------------------
+// K4 v2: row-span voxelizer (default).  DESIGN.md "Kernels / K4 span".
+// Inside a tile row (y,z) every half-space G_k(x) = r_k + mx_k*x >= 0 is a half-line in x, so the
+// row's solid set is ONE interval [lower, upper].  Each plane is stored as a function Q that is
+// non-increasing in x and whose non-negative set {x : Q(x) >= 0} is
+//   hi-type (mx_G < 0): Q = G                     -> x <= b,  b = max{x : G(x) >= 0}
+//   lo-type (mx_G > 0): Q = -G - 1  (G <= -1)     -> x <= b  <=> G(x) < 0, so the half-space is x >= b+1
+//   mx_G == 0:          Q = 64*G + 63 - x (hi)    -> equivalent on x in [0,63] for integer G
+// b = floor of the real crossing.  A float PROPOSES c0 = rint(Q_row * (1/|mx|)), clamped to [-1,32];
+// the INTEGER value Q(c0) decides: b = c0 if Q(c0) >= 0 else c0-1.  The proposal is within 0.5 of the
+// crossing whenever that lies in [-1.5,32.5] (relative float error <= 2^-21), so b is exact there, and
+// saturates correctly outside.  All Q(x), x in [-1,32], fit int32 (checked in int64 at setup).
+// ------------------------------------------------------------------------------------------
+enum { SREC_W = 36, KIND_SPAN = 0 };  // record stride 36 words: int4-aligned, conflict-free 128-bit stores
+// record words: [0..3] mx  [4..7] my  [8..11] mz  [12..15] g0 (at row y0,z0)  [16..19] 1/|mx| (float bits)
+//               [20] x0-1  [21] x1  [22] ny  [23] nrows  [24] y0 | z0<<8 | nlo<<16 | kind<<24  [25] div magic
+//               [26] tet id  [27] packed local box
+
+__device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0, int Y0, int Z0, int* rec) {
+    Tet q = load_tet(p, t);
+    Planes P;
+    tet_planes(p, q, X0, Y0, Z0, P);
+    const u32 box = local_box(p, q, X0, Y0, Z0);
+    const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
+    const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
+    bool fits = true;
+    int nlo = 0;
+    i64 qx[4], qy[4], qz[4], q0[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        i64 mx = P.mx[k], my = P.my[k], mz = P.mz[k], g0 = P.g0[k];
+        if (mx > 0) { mx = -mx; my = -my; mz = -mz; g0 = -g0 - 1; }
+        else if (mx == 0) {
+            // 64*G + 63 - x: guard the scaling itself against int64 overflow (then it cannot fit anyway)
+            if (iabs64(my) > (1ll << 40) || iabs64(mz) > (1ll << 40) || iabs64(g0) > (1ll << 40)) fits = false;
+            mx = -1; my *= 64; mz *= 64; g0 = g0 * 64 + 63;
+        }
+        i64 bound = iabs64(g0) + 33 * (iabs64(mx) + iabs64(my) + iabs64(mz));
+        fits = fits && (bound < 0x7FFFFF00ll);
+        qx[k] = mx; qy[k] = my; qz[k] = mz; q0[k] = g0 + my * y0 + mz * z0;
+        nlo += (P.mx[k] > 0);
+    }
+    const int ny = y1 - y0 + 1, nrows = ny * (z1 - z0 + 1);
+    if (fits) {
+        int lo_seen = 0, hi_seen = 0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const bool is_lo = P.mx[k] > 0;
+            const int pos = is_lo ? lo_seen : nlo + hi_seen;
+            lo_seen += is_lo; hi_seen += !is_lo;
+            rec[pos] = (int)qx[k];
+            rec[4 + pos] = (int)qy[k];
+            rec[8 + pos] = (int)qz[k];
+            rec[12 + pos] = (int)q0[k];
+            rec[16 + pos] = __float_as_int(1.0f / (float)(-qx[k]));
+        }
+    }
+    int4 tail;
+    tail.x = x0 - 1; tail.y = x1; tail.z = ny; tail.w = nrows;
+    *reinterpret_cast<int4*>(rec + 20) = tail;
+    int4 tail2;
+    tail2.x = y0 | (z0 << 8) | (nlo << 16) | ((fits ? KIND_SPAN : KIND_LARGE) << 24);
+    tail2.y = (int)((65536u + ny - 1) / ny);
+    tail2.z = (int)t;
+    tail2.w = (int)box;
+    *reinterpret_cast<int4*>(rec + 24) = tail2;
+}
+
+// b = max{x in [-1,32] : Q(x) >= 0} (or -2 if none), Q(x) = r + mx*x, mx < 0
+__device__ __forceinline__ int span_bound(int r, int mx, float inv) {
+    float xf = __int2float_rn(r) * inv;
+    xf = fminf(fmaxf(xf, -1.0f), 32.0f);
+    const int c0 = __float2int_rn(xf);
+    const int v = r + mx * c0;
+    return c0 + (v >> 31);
+}
+
+template <int NLO>
+__device__ __forceinline__ void raster_span(const int* rec, u32* img, int lane, int ty_log) {
+    const int4 MX = *reinterpret_cast<const int4*>(rec);
+    const int4 MY = *reinterpret_cast<const int4*>(rec + 4);
+    const int4 MZ = *reinterpret_cast<const int4*>(rec + 8);
+    const int4 G0 = *reinterpret_cast<const int4*>(rec + 12);
+    const float4 IV = *reinterpret_cast<const float4*>(rec + 16);
+    const int4 A = *reinterpret_cast<const int4*>(rec + 20);  // x0-1, x1, ny, nrows
+    const int4 B = *reinterpret_cast<const int4*>(rec + 24);
+    const int y0 = B.x & 255, z0 = (B.x >> 8) & 255;
+    const u32 dinv = (u32)B.y;
+    for (int r = lane; r < A.w; r += 32) {
+        const int zz = (int)(((u32)r * dinv) >> 16);
+        const int yy = r - zz * A.z;
+        const int b0 = span_bound(G0.x + MY.x * yy + MZ.x * zz, MX.x, IV.x);
+        const int b1 = span_bound(G0.y + MY.y * yy + MZ.y * zz, MX.y, IV.y);
+        const int b2 = span_bound(G0.z + MY.z * yy + MZ.z * zz, MX.z, IV.z);
+        const int b3 = span_bound(G0.w + MY.w * yy + MZ.w * zz, MX.w, IV.w);
+        int lower, upper;  // lower is (first solid x) - 1
+        if (NLO == 1) { lower = max(A.x, b0); upper = min(min(A.y, b1), min(b2, b3)); }
+        else if (NLO == 2) { lower = max(A.x, max(b0, b1)); upper = min(A.y, min(b2, b3)); }
+        else { lower = max(max(A.x, b0), max(b1, b2)); upper = min(A.y, b3); }
+        const int n = upper - lower;  // number of solid voxels
+        if (n > 0) {
+            const u32 word = (0xFFFFFFFFu >> (32 - n)) << (lower + 1);
+            atomicOr(img + img_idx(y0 + yy, z0 + zz, ty_log), word);
+        }
+    }
+}
+
+template <int NT>
+__global__ void __launch_bounds__(NT) k4_span(Params p, const u32* __restrict__ offsets, const u32* __restrict__ list,
+                                              u32* __restrict__ bits, u32* __restrict__ hdr) {
+    __shared__ u32 img[1024];
+    __shared__ __align__(16) int rec[NT][SREC_W];
+    __shared__ u32 s_large;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = NT / 32;
+    const u32 b = blockIdx.x;
+    const u32 bx = b % p.nbx;
+    u32 rest = b / p.nbx;
+    const u32 by = rest % p.nby;
+    rest /= p.nby;
+    const u32 bz = rest % p.nbz;
+    const u32 m = rest / p.nbz;
+    const int X0 = bx << 5, Y0 = by << p.ty_log, Z0 = bz << p.tz_log;
+    const int rows = 1 << (p.ty_log + p.tz_log);
+    for (int i = tid; i < rows; i += NT) img[i] = 0;
+    if (tid == 0) s_large = 0;
+    const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
+    for (u32 base = beg; base < end; base += NT) {
+        __syncthreads();
+        const int n = min((u32)NT, end - base);
+        if (tid < n) setup_span_record(p, list[base + tid], X0, Y0, Z0, rec[tid]);
+        __syncthreads();
+        for (int i = warp; i < n; i += NW) {
+            const int* r = rec[i];
+            const int info = r[24];
+            const int nlo = (info >> 16) & 255;
+            if ((info >> 24) == KIND_SPAN) {
+                if (nlo == 2) raster_span<2>(r, img, lane, p.ty_log);
+                else if (nlo == 1) raster_span<1>(r, img, lane, p.ty_log);
+                else if (nlo == 3) raster_span<3>(r, img, lane, p.ty_log);
+                // nlo == 0 or 4: some half-space excludes a whole x-direction: cannot happen for a
+                // non-degenerate tet (its four face normals sum to zero); nothing to draw
+            } else {
+                raster_large(p, (u32)r[26], (u32)r[27], X0, Y0, Z0, img, lane);
+                if (lane == 0) atomicAdd(&s_large, 1u);
+            }
+        }
+    }
+    __syncthreads();
+    const int TY = 1 << p.ty_log;
+    for (int i = tid; i < rows; i += NT) {
+        const int z = i >> p.ty_log, y = i & (TY - 1);
+        const int gy = Y0 + y, gz = Z0 + z;
+        if (gy < p.ny && gz < p.nz)
+            bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[img_idx(y, z, p.ty_log)];
+    }
+    if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
+}
+
+// ------------------------------------------------------------------------------------------
 // validation and probes
 // ------------------------------------------------------------------------------------------
 __global__ void k_validate(Params p, u32* hdr) {
@@ -760,7 +919,8 @@ extern "C" int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_
         k3_scatter<<<blocks, 256, 0, st>>>(p, range, cursor, list, hdr);
     }
     if (ev) CK(cudaEventRecord(ev[3], st));
-    k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
+    if (ctx->variant == 1) k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
+    else k4_span<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
     CK(cudaGetLastError());
     if (ev) {
         CK(cudaEventRecord(ev[4], st));

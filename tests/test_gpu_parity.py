@@ -82,6 +82,13 @@ def test_parity_is_tile_independent(name, tile):
     assert_same(gpu_voxelize(m, tile=tile), cpu_voxelize(m), f"{name} tile={tile}")
 
 
+@pytest.mark.parametrize("name", ["cfg1_sphere", "cfg2", "cfg4_small_drop3", "giant128_sphere", "giant256_nojit"])
+def test_parity_walker_variant(name):
+    # variant 1 = the x-walk voxelizer kept for A/B comparison; same bits
+    m = CASES[name]()
+    assert_same(gpu_voxelize(m, variant=1), cpu_voxelize(m), f"{name} variant=1")
+
+
 def test_estimated_workspace_path():
     m = CASES["cfg2"]()
     assert_same(gpu_voxelize(m, exact_plan=False), cpu_voxelize(m), "cfg2 without vox_plan")
