@@ -591,8 +591,8 @@ __device__ __forceinline__ void raster_span(const int* rec, u32* img, int lane, 
     }
 }
 
-template <int NT>
-__global__ void __launch_bounds__(NT) k4_span(Params p, const u32* __restrict__ offsets, const u32* __restrict__ list,
+template <int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restrict__ offsets, const u32* __restrict__ list,
                                               u32* __restrict__ bits, u32* __restrict__ hdr) {
     __shared__ u32 img[1024];
     __shared__ __align__(16) int rec[NT][SREC_W];
@@ -920,7 +920,11 @@ extern "C" int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_
     }
     if (ev) CK(cudaEventRecord(ev[3], st));
     if (ctx->variant == 1) k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
-    else k4_span<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
+    else if (ctx->variant == 2) k4_span<256, 3><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
+    else if (ctx->variant == 3) k4_span<256, 4><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
+    else if (ctx->variant == 4) k4_span<128, 8><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr);
+    else if (ctx->variant == 5) k4_span<128, 6><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr);
+    else k4_span<256, 2><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
     CK(cudaGetLastError());
     if (ev) {
         CK(cudaEventRecord(ev[4], st));
