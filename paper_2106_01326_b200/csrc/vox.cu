@@ -304,10 +304,6 @@ __device__ __forceinline__ void tet_planes(const Params& p, const Tet& q, int X0
 
 __device__ __forceinline__ i64 iabs64(i64 v) { return v < 0 ? -v : v; }
 
-// smem image index of tile row (y,z); skewed so that a tet's rows spread over banks
-__device__ __forceinline__ int img_idx(int y, int z, int ty_log) {
-    return (z << ty_log) + ((y + 11 * z) & ((1 << ty_log) - 1));
-}
 
 enum { REC_W = 18, KIND_FAST = 0, KIND_LARGE = 1 };
 // record: [0..3] mx, [4..7] my, [8..11] mz, [12..15] g0, [16] box, [17] kind | (for LARGE: [0] = tet id)
@@ -359,7 +355,7 @@ __device__ __forceinline__ void setup_record(const Params& p, u32 t, int X0, int
 
 // Fast path: all four G fit int32 over the whole tile.  Lanes = rows (y,z) of the
 // tet's local box; each lane walks its row's x-span and builds the row word.
-__device__ __forceinline__ void raster_fast(const int* rec, u32* img, int lane, int ty_log) {
+__device__ __forceinline__ void raster_fast(const int* rec, u32* img, int lane, int img_stride) {
     const u32 box = (u32)rec[16];
     const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
     const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
@@ -391,14 +387,15 @@ __device__ __forceinline__ void raster_fast(const int* rec, u32* img, int lane, 
             }
         }
         const u32 word = (~out & wmask) << x0;
-        if (word) atomicOr(img + img_idx(y, z, ty_log), word);
+        if (word) atomicOr(img + z * img_stride + y, word);
     }
 }
 
 // Large path (K5): planes do not fit int32 on this tile.  The whole warp works on one
 // (tet, tile): exact classification of the local box, then a 64-bit ballot rasteriser
 // with lanes = the 32 x positions of a row word.
-__device__ __noinline__ void raster_large(const Params& p, u32 t, u32 box, int X0, int Y0, int Z0, u32* img, int lane) {
+__device__ __noinline__ void raster_large(const Params& p, u32 t, u32 box, int X0, int Y0, int Z0, u32* img, int lane,
+                                          int img_stride) {
     Tet q = load_tet(p, t);
     Planes P;
     tet_planes(p, q, X0, Y0, Z0, P);
@@ -421,7 +418,7 @@ __device__ __noinline__ void raster_large(const Params& p, u32 t, u32 box, int X
         const int nrows = ny * (z1 - z0 + 1);
         for (int r = lane; r < nrows; r += 32) {
             int zz = r / ny;
-            atomicOr(img + img_idx(y0 + r - zz * ny, z0 + zz, p.ty_log), xmask);
+            atomicOr(img + (z0 + zz) * img_stride + y0 + r - zz * ny, xmask);
         }
         return;
     }
@@ -432,7 +429,7 @@ __device__ __noinline__ void raster_large(const Params& p, u32 t, u32 box, int X
         i64 r2 = c2 + P.mz[2] * z + P.my[2] * y0, r3 = c3 + P.mz[3] * z + P.my[3] * y0;
         for (int y = y0; y <= y1; ++y) {
             u32 word = __ballot_sync(0xFFFFFFFFu, (r0 | r1 | r2 | r3) >= 0) & xmask;
-            if (lane == 0 && word) atomicOr(img + img_idx(y, z, p.ty_log), word);
+            if (lane == 0 && word) atomicOr(img + z * img_stride + y, word);
             r0 += P.my[0]; r1 += P.my[1]; r2 += P.my[2]; r3 += P.my[3];
         }
     }
@@ -441,7 +438,7 @@ __device__ __noinline__ void raster_large(const Params& p, u32 t, u32 box, int X
 template <int NT>
 __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__ offsets, const u32* __restrict__ list,
                                                u32* __restrict__ bits, u32* __restrict__ hdr) {
-    __shared__ u32 img[1024];
+    __shared__ u32 img[32 * 43];
     __shared__ __align__(16) int rec[NT][REC_W + 2];  // row = 20 words: int4-aligned
     __shared__ u32 s_large;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -455,7 +452,8 @@ __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__
     const u32 m = rest / p.nbz;
     const int X0 = bx << 5, Y0 = by << p.ty_log, Z0 = bz << p.tz_log;
     const int rows = 1 << (p.ty_log + p.tz_log);
-    for (int i = tid; i < rows; i += NT) img[i] = 0;
+    const int img_stride = (1 << p.ty_log) + 11;
+    for (int i = tid; i < (img_stride << p.tz_log); i += NT) img[i] = 0;
     if (tid == 0) s_large = 0;
     const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
     for (u32 base = beg; base < end; base += NT) {
@@ -466,9 +464,9 @@ __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__
         for (int i = warp; i < n; i += NW) {
             const int* r = rec[i];
             if (r[17] == KIND_FAST) {
-                raster_fast(r, img, lane, p.ty_log);
+                raster_fast(r, img, lane, img_stride);
             } else {
-                raster_large(p, (u32)r[0], (u32)r[16], X0, Y0, Z0, img, lane);
+                raster_large(p, (u32)r[0], (u32)r[16], X0, Y0, Z0, img, lane, img_stride);
                 if (lane == 0) atomicAdd(&s_large, 1u);
             }
         }
@@ -479,7 +477,7 @@ __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__
         const int z = i >> p.ty_log, y = i & (TY - 1);
         const int gy = Y0 + y, gz = Z0 + z;
         if (gy < p.ny && gz < p.nz)
-            bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[img_idx(y, z, p.ty_log)];
+            bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[z * img_stride + y];
     }
     if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
 }
@@ -497,104 +495,138 @@ __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__
 // crossing whenever that lies in [-1.5,32.5] (relative float error <= 2^-21), so b is exact there, and
 // saturates correctly outside.  All Q(x), x in [-1,32], fit int32 (checked in int64 at setup).
 // ------------------------------------------------------------------------------------------
-enum { SREC_W = 36, KIND_SPAN = 0 };  // record stride 36 words: int4-aligned, conflict-free 128-bit stores
+enum { SREC_W = 36, KIND_SPAN = 0, IMG_SKEW = 11 };  // record stride 36 words: int4-aligned
 // record words: [0..3] mx  [4..7] my  [8..11] mz  [12..15] g0 (at row y0,z0)  [16..19] 1/|mx| (float bits)
-//               [20] x0-1  [21] x1  [22] ny  [23] nrows  [24] y0 | z0<<8 | nlo<<16 | kind<<24  [25] div magic
-//               [26] tet id  [27] packed local box
+//               [20] x0-1  [21] x1  [22] ny  [23] nrows  [24] image index of row (y0,z0)
+//               [25] div magic  [26] nlo | kind<<8  [27] tet id  [28] packed local box
+// image: row (y,z) of the tile lives at img[z*(TY+IMG_SKEW) + y] (skew spreads a tet's rows over banks)
 
-__device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0, int Y0, int Z0, int* rec) {
-    Tet q = load_tet(p, t);
-    Planes P;
-    tet_planes(p, q, X0, Y0, Z0, P);
-    const u32 box = local_box(p, q, X0, Y0, Z0);
-    const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
-    const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
-    bool fits = true;
-    int nlo = 0;
-    i64 qx[4], qy[4], qz[4], q0[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        i64 mx = P.mx[k], my = P.my[k], mz = P.mz[k], g0 = P.g0[k];
-        if (mx > 0) { mx = -mx; my = -my; mz = -mz; g0 = -g0 - 1; }
-        else if (mx == 0) {
-            // 64*G + 63 - x: guard the scaling itself against int64 overflow (then it cannot fit anyway)
-            if (iabs64(my) > (1ll << 40) || iabs64(mz) > (1ll << 40) || iabs64(g0) > (1ll << 40)) fits = false;
-            mx = -1; my *= 64; mz *= 64; g0 = g0 * 64 + 63;
-        }
-        i64 bound = iabs64(g0) + 33 * (iabs64(mx) + iabs64(my) + iabs64(mz));
-        fits = fits && (bound < 0x7FFFFF00ll);
-        qx[k] = mx; qy[k] = my; qz[k] = mz; q0[k] = g0 + my * y0 + mz * z0;
-        nlo += (P.mx[k] > 0);
+// One plane of the span record.  (nx,ny,nz) = sigma*N (int32, exact), (rx,ry,rz) = Q - P0.
+// G(j) = floor(C/g) - sum_a (sigma*N_a*s_a) j_a, C = sigma*N.(Q-P0)
+__device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, int nx, int ny, int nz, int rx, int ry,
+                                           int rz, int y0, int z0) {
+    const i64 C = (i64)nx * rx + (i64)ny * ry + (i64)nz * rz;
+    i64 g0 = C >> p.g_shift;
+    i64 mx = -(i64)nx * p.sx, my = -(i64)ny * p.sy, mz = -(i64)nz * p.sz;
+    bool ok = true;
+    if (mx > 0) { mx = -mx; my = -my; mz = -mz; g0 = -g0 - 1; }  // lo-type: Q = -G - 1
+    else if (mx == 0) {                                          // Q = 64*G + 63 - x
+        ok = (iabs64(g0) < (1ll << 40));
+        mx = -1; my *= 64; mz *= 64; g0 = g0 * 64 + 63;
     }
-    const int ny = y1 - y0 + 1, nrows = ny * (z1 - z0 + 1);
-    if (fits) {
-        int lo_seen = 0, hi_seen = 0;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const bool is_lo = P.mx[k] > 0;
-            const int pos = is_lo ? lo_seen : nlo + hi_seen;
-            lo_seen += is_lo; hi_seen += !is_lo;
-            rec[pos] = (int)qx[k];
-            rec[4 + pos] = (int)qy[k];
-            rec[8 + pos] = (int)qz[k];
-            rec[12 + pos] = (int)q0[k];
-            rec[16 + pos] = __float_as_int(1.0f / (float)(-qx[k]));
-        }
-    }
-    int4 tail;
-    tail.x = x0 - 1; tail.y = x1; tail.z = ny; tail.w = nrows;
-    *reinterpret_cast<int4*>(rec + 20) = tail;
-    int4 tail2;
-    tail2.x = y0 | (z0 << 8) | (nlo << 16) | ((fits ? KIND_SPAN : KIND_LARGE) << 24);
-    tail2.y = (int)((65536u + ny - 1) / ny);
-    tail2.z = (int)t;
-    tail2.w = (int)box;
-    *reinterpret_cast<int4*>(rec + 24) = tail2;
+    const i64 bound = iabs64(g0) + 130 * iabs64(mx) + 32 * (iabs64(my) + iabs64(mz));
+    ok = ok && (bound < 0x7FFFFF00ll);
+    rec[pos] = (int)mx;
+    rec[4 + pos] = (int)my;
+    rec[8 + pos] = (int)mz;
+    rec[12 + pos] = (int)(g0 + my * y0 + mz * z0);
+    rec[16 + pos] = __float_as_int(1.0f / (float)(-(int)mx));
+    return ok;
 }
 
-// b = max{x in [-1,32] : Q(x) >= 0} (or -2 if none), Q(x) = r + mx*x, mx < 0
+// thread-per-(tet,tile) setup in 32-bit arithmetic.  Needs the tet's lattice bbox extent < 2^15 per
+// axis (all edge components < 2^15, so every cross-product component is < 2^31) and g a power of two;
+// anything else, or plane values that do not fit int32 on the tile, is handed to the int64 large path.
+__device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0, int Y0, int Z0, int img_stride,
+                                                  int* rec) {
+    const Tet q = load_tet(p, t);
+    const int lox = min(min(q.ax, q.bx), min(q.cx, q.dx)), hix = max(max(q.ax, q.bx), max(q.cx, q.dx));
+    const int loy = min(min(q.ay, q.by), min(q.cy, q.dy)), hiy = max(max(q.ay, q.by), max(q.cy, q.dy));
+    const int loz = min(min(q.az, q.bz), min(q.cz, q.dz)), hiz = max(max(q.az, q.bz), max(q.cz, q.dz));
+    // local closed voxel box (same rounding as K1's axis_range), clipped to the tile
+    const int TY = 1 << p.ty_log, TZ = 1 << p.tz_log;
+    int x0 = -floor_div_i(p.hx - 2 * lox, 2 * p.hx), x1 = floor_div_i(2 * hix - p.hx, 2 * p.hx);
+    int y0 = -floor_div_i(p.hy - 2 * loy, 2 * p.hy), y1 = floor_div_i(2 * hiy - p.hy, 2 * p.hy);
+    int z0 = -floor_div_i(p.hz - 2 * loz, 2 * p.hz), z1 = floor_div_i(2 * hiz - p.hz, 2 * p.hz);
+    x0 = max(x0 - X0, 0); x1 = min(min(x1, p.nx - 1) - X0, 31);
+    y0 = max(y0 - Y0, 0); y1 = min(min(y1, p.ny - 1) - Y0, TY - 1);
+    z0 = max(z0 - Z0, 0); z1 = min(min(z1, p.nz - 1) - Z0, TZ - 1);
+    const int ny = y1 - y0 + 1, nrows = ny * (z1 - z0 + 1);
+    bool ok = (((hix - lox) | (hiy - loy) | (hiz - loz)) < 32768) && (p.g_shift >= 0);
+    int nlo = 0;
+    if (ok) {
+        const int ux = q.bx - q.ax, uy = q.by - q.ay, uz = q.bz - q.az;
+        const int vx = q.cx - q.ax, vy = q.cy - q.ay, vz = q.cz - q.az;
+        const int wx = q.dx - q.ax, wy = q.dy - q.ay, wz = q.dz - q.az;
+        // N_b = v x w, N_c = u x w, N_d = u x v, N_a = (v-u) x (w-u) = N_b - N_c + N_d
+        const int nbx = vy * wz - vz * wy, nby = vz * wx - vx * wz, nbz = vx * wy - vy * wx;
+        const int ncx = uy * wz - uz * wy, ncy = uz * wx - ux * wz, ncz = ux * wy - uy * wx;
+        const int ndx = uy * vz - uz * vy, ndy = uz * vx - ux * vz, ndz = ux * vy - uy * vx;
+        const int nax = (int)((u32)nbx - (u32)ncx + (u32)ndx), nay = (int)((u32)nby - (u32)ncy + (u32)ndy);
+        const int naz = (int)((u32)nbz - (u32)ncz + (u32)ndz);
+        const i64 det = (i64)ux * nbx + (i64)uy * nby + (i64)uz * nbz;  // 6V = u.(v x w) != 0 (K1 culled 0)
+        const int s = det > 0 ? 1 : -1;
+        // sigma = (s, -s, s, -s): F = (s*D_a, -s*D_b, s*D_c, -s*D_d) >= 0 inside
+        const int p0x = p.hx * X0 + (p.hx >> 1), p0y = p.hy * Y0 + (p.hy >> 1), p0z = p.hz * Z0 + (p.hz >> 1);
+        const int arx = q.ax - p0x, ary = q.ay - p0y, arz = q.az - p0z;
+        const int brx = q.bx - p0x, bry = q.by - p0y, brz = q.bz - p0z;
+        // m_x = -sigma*N_x*sx > 0  <=>  lo-type
+        const bool l0 = s * nax < 0, l1 = s * nbx > 0, l2 = s * ncx < 0, l3 = s * ndx > 0;
+        nlo = (int)l0 + (int)l1 + (int)l2 + (int)l3;
+        const int pos0 = l0 ? 0 : nlo;
+        const int pos1 = l1 ? (int)l0 : nlo + (int)!l0;
+        const int pos2 = l2 ? (int)l0 + (int)l1 : nlo + (int)!l0 + (int)!l1;
+        const int pos3 = l3 ? nlo - 1 : 3;
+        ok = span_plane(p, rec, pos0, s * nax, s * nay, s * naz, brx, bry, brz, y0, z0) && ok;
+        ok = span_plane(p, rec, pos1, -s * nbx, -s * nby, -s * nbz, arx, ary, arz, y0, z0) && ok;
+        ok = span_plane(p, rec, pos2, s * ncx, s * ncy, s * ncz, arx, ary, arz, y0, z0) && ok;
+        ok = span_plane(p, rec, pos3, -s * ndx, -s * ndy, -s * ndz, arx, ary, arz, y0, z0) && ok;
+    }
+    int4 a;
+    a.x = x0 - 1; a.y = x1; a.z = ny; a.w = nrows;
+    *reinterpret_cast<int4*>(rec + 20) = a;
+    int4 b;
+    b.x = z0 * img_stride + y0;
+    b.y = (int)((65536u + ny - 1) / ny);
+    b.z = nlo | ((ok ? KIND_SPAN : KIND_LARGE) << 8);
+    b.w = (int)t;
+    *reinterpret_cast<int4*>(rec + 24) = b;
+    rec[28] = (int)pack_box(x0, x1, y0, y1, z0, z1);
+}
+
+// b = max{x in [-128,127] : Q(x) >= 0} (one less if none), Q(x) = r + mx*x, mx < 0.
+// F2I.S8 saturates, which bounds |mx*c0| (the int32 fit check at setup covers |x| <= 130).
 __device__ __forceinline__ int span_bound(int r, int mx, float inv) {
-    float xf = __int2float_rn(r) * inv;
-    xf = fminf(fmaxf(xf, -1.0f), 32.0f);
-    const int c0 = __float2int_rn(xf);
+    const float xf = __int2float_rn(r) * inv;
+    int c0;
+    asm("cvt.rni.s8.f32 %0, %1;" : "=r"(c0) : "f"(xf));
     const int v = r + mx * c0;
     return c0 + (v >> 31);
 }
 
 template <int NLO>
-__device__ __forceinline__ void raster_span(const int* rec, u32* img, int lane, int ty_log) {
+__device__ __forceinline__ void raster_span(const int* rec, u32* img, int lane, int img_stride) {
     const int4 MX = *reinterpret_cast<const int4*>(rec);
     const int4 MY = *reinterpret_cast<const int4*>(rec + 4);
     const int4 MZ = *reinterpret_cast<const int4*>(rec + 8);
     const int4 G0 = *reinterpret_cast<const int4*>(rec + 12);
     const float4 IV = *reinterpret_cast<const float4*>(rec + 16);
     const int4 A = *reinterpret_cast<const int4*>(rec + 20);  // x0-1, x1, ny, nrows
-    const int4 B = *reinterpret_cast<const int4*>(rec + 24);
-    const int y0 = B.x & 255, z0 = (B.x >> 8) & 255;
-    const u32 dinv = (u32)B.y;
+    const int2 B = *reinterpret_cast<const int2*>(rec + 24);  // image index of row (y0,z0), div magic
     for (int r = lane; r < A.w; r += 32) {
-        const int zz = (int)(((u32)r * dinv) >> 16);
+        const int zz = (int)(((u32)r * (u32)B.y) >> 16);
         const int yy = r - zz * A.z;
         const int b0 = span_bound(G0.x + MY.x * yy + MZ.x * zz, MX.x, IV.x);
         const int b1 = span_bound(G0.y + MY.y * yy + MZ.y * zz, MX.y, IV.y);
         const int b2 = span_bound(G0.z + MY.z * yy + MZ.z * zz, MX.z, IV.z);
         const int b3 = span_bound(G0.w + MY.w * yy + MZ.w * zz, MX.w, IV.w);
-        int lower, upper;  // lower is (first solid x) - 1
+        int lower, upper;  // lower = (first solid x) - 1
         if (NLO == 1) { lower = max(A.x, b0); upper = min(min(A.y, b1), min(b2, b3)); }
         else if (NLO == 2) { lower = max(A.x, max(b0, b1)); upper = min(A.y, min(b2, b3)); }
         else { lower = max(max(A.x, b0), max(b1, b2)); upper = min(A.y, b3); }
-        const int n = upper - lower;  // number of solid voxels
+        const int n = upper - lower;  // number of solid voxels in the row
         if (n > 0) {
             const u32 word = (0xFFFFFFFFu >> (32 - n)) << (lower + 1);
-            atomicOr(img + img_idx(y0 + yy, z0 + zz, ty_log), word);
+            atomicOr(img + B.x + zz * img_stride + yy, word);
         }
     }
 }
 
 template <int NT, int MINB>
-__global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restrict__ offsets, const u32* __restrict__ list,
-                                              u32* __restrict__ bits, u32* __restrict__ hdr) {
-    __shared__ u32 img[1024];
+__global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restrict__ offsets,
+                                                    const u32* __restrict__ list, u32* __restrict__ bits,
+                                                    u32* __restrict__ hdr) {
+    __shared__ u32 img[32 * (32 + IMG_SKEW)];
     __shared__ __align__(16) int rec[NT][SREC_W];
     __shared__ u32 s_large;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -607,38 +639,39 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
     const u32 bz = rest % p.nbz;
     const u32 m = rest / p.nbz;
     const int X0 = bx << 5, Y0 = by << p.ty_log, Z0 = bz << p.tz_log;
-    const int rows = 1 << (p.ty_log + p.tz_log);
-    for (int i = tid; i < rows; i += NT) img[i] = 0;
+    const int TY = 1 << p.ty_log, img_stride = TY + IMG_SKEW;
+    const int img_words = img_stride << p.tz_log;
+    for (int i = tid; i < img_words; i += NT) img[i] = 0;
     if (tid == 0) s_large = 0;
     const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
     for (u32 base = beg; base < end; base += NT) {
         __syncthreads();
         const int n = min((u32)NT, end - base);
-        if (tid < n) setup_span_record(p, list[base + tid], X0, Y0, Z0, rec[tid]);
+        if (tid < n) setup_span_record(p, list[base + tid], X0, Y0, Z0, img_stride, rec[tid]);
         __syncthreads();
         for (int i = warp; i < n; i += NW) {
             const int* r = rec[i];
-            const int info = r[24];
-            const int nlo = (info >> 16) & 255;
-            if ((info >> 24) == KIND_SPAN) {
-                if (nlo == 2) raster_span<2>(r, img, lane, p.ty_log);
-                else if (nlo == 1) raster_span<1>(r, img, lane, p.ty_log);
-                else if (nlo == 3) raster_span<3>(r, img, lane, p.ty_log);
-                // nlo == 0 or 4: some half-space excludes a whole x-direction: cannot happen for a
-                // non-degenerate tet (its four face normals sum to zero); nothing to draw
+            const int info = r[26];
+            if ((info >> 8) == KIND_SPAN) {
+                const int nlo = info & 255;
+                if (nlo == 2) raster_span<2>(r, img, lane, img_stride);
+                else if (nlo == 1) raster_span<1>(r, img, lane, img_stride);
+                else if (nlo == 3) raster_span<3>(r, img, lane, img_stride);
+                // nlo == 0 or 4 cannot happen for a non-degenerate tet (the four sigma*N sum to zero
+                // and planes with N_x == 0 count as hi-type): nothing to draw
             } else {
-                raster_large(p, (u32)r[26], (u32)r[27], X0, Y0, Z0, img, lane);
+                raster_large(p, (u32)r[27], (u32)r[28], X0, Y0, Z0, img, lane, img_stride);
                 if (lane == 0) atomicAdd(&s_large, 1u);
             }
         }
     }
     __syncthreads();
-    const int TY = 1 << p.ty_log;
+    const int rows = 1 << (p.ty_log + p.tz_log);
     for (int i = tid; i < rows; i += NT) {
         const int z = i >> p.ty_log, y = i & (TY - 1);
         const int gy = Y0 + y, gz = Z0 + z;
         if (gy < p.ny && gz < p.nz)
-            bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[img_idx(y, z, p.ty_log)];
+            bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[z * img_stride + y];
     }
     if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
 }
@@ -920,11 +953,9 @@ extern "C" int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_
     }
     if (ev) CK(cudaEventRecord(ev[3], st));
     if (ctx->variant == 1) k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
-    else if (ctx->variant == 2) k4_span<256, 3><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
+    else if (ctx->variant == 2) k4_span<256, 2><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
     else if (ctx->variant == 3) k4_span<256, 4><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
-    else if (ctx->variant == 4) k4_span<128, 8><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr);
-    else if (ctx->variant == 5) k4_span<128, 6><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr);
-    else k4_span<256, 2><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
+    else k4_span<128, 8><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr);  // 64 regs, 32 warps/SM
     CK(cudaGetLastError());
     if (ev) {
         CK(cudaEventRecord(ev[4], st));
