@@ -73,6 +73,42 @@ def candidate_samples(m):
     return total
 
 
+def rank_seed(workload, rank):
+    """Replicas: rank r voxelizes its own mesh of the same recipe, seed = default seed + r."""
+    from meshgen.kuhn import _CONFIGS
+
+    return _CONFIGS[workload][1] + rank
+
+
+def reduce_over_ranks(dist, ms, samples, tets, device):
+    """(max over ranks of the device time, sum over ranks of the work).  No data-path collective:
+    this is the only communication of a multi-rank run."""
+    if dist is None:
+        return float(ms), float(samples), float(tets)
+    import torch
+
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    w = torch.tensor([float(samples), float(tets)], dtype=torch.float64, device=device)
+    dist.all_reduce(w, op=dist.ReduceOp.SUM)
+    return float(t[0]), float(w[0]), float(w[1])
+
+
+def ncu_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, from the
+    committed ncu --set full capture (profiles/traffic.csv names the capture); None if absent."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        best = None
+        for ln in open(path).read().splitlines():
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) >= 5 and f[0] == workload and f[1] == kernel:
+                best = {"bytes": float(f[2]) + float(f[3]), "source": "profiles/" + f[4]}
+        return best
+    except OSError:
+        return None
+
+
 class ClockSampler:
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
@@ -243,12 +279,7 @@ def run_b200(args):
 
     # replicas: rank r voxelizes its own mesh of the same recipe (default seed + r)
     base = meshgen.make_config(args.workload, None) if rank == 0 else None
-    if rank == 0:
-        m = base
-    else:
-        from meshgen.kuhn import _CONFIGS
-
-        m = meshgen.make_config(args.workload, _CONFIGS[args.workload][1] + rank)
+    m = base if rank == 0 else meshgen.make_config(args.workload, rank_seed(args.workload, rank))
     samples = candidate_samples(m)
 
     stream = torch.cuda.Stream()
@@ -292,13 +323,7 @@ def run_b200(args):
             popcount = int(np.unpackbits(out.cpu().numpy().view(np.uint8)).sum())
 
         # max over ranks of the device time; sum over ranks of the work
-        tmax, ssum, tsum = ms_total, float(samples), float(m.T)
-        if dist is not None:
-            t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            w = torch.tensor([float(samples), float(m.T)], dtype=torch.float64, device="cuda")
-            dist.all_reduce(w, op=dist.ReduceOp.SUM)
-            tmax, ssum, tsum = float(t[0]), float(w[0]), float(w[1])
+        tmax, ssum, tsum = reduce_over_ranks(dist, ms_total, samples, m.T, "cuda")
         sec = tmax * 1e-3
         value = ssum * args.steps / sec / 1e9
 
@@ -325,10 +350,7 @@ def run_b200(args):
             torch.cuda.synchronize()
             wall = time.perf_counter() - t0
             e2e_ms = max(f0.elapsed_time(f1), wall * 1e3)
-            if dist is not None:
-                t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                e2e_ms = float(t[0])
+            e2e_ms = reduce_over_ranks(dist, e2e_ms, 0, 0, "cuda")[0]
             h2d = hv.numel() * 4 + ht.numel() * 4 + (ho.numel() * 8 if ho is not None else 0)
             d2h = hout.numel() * 4 + 256  # grid + the status header
             e2e = {"value": ssum * args.e2e_steps / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
@@ -363,9 +385,10 @@ def run_b200(args):
         hbm_peak = peaks.get("hbm_gbs", 6650.0)
         min_bytes = 16.0 * m.T + 12.0 * m.V + 4.0 * vz.grid_words
         k4_bytes = 4.0 * vz.grid_words + pairs * (4.0 + 16.0 + 48.0)  # grid + per pair: id, tet, 4 verts
+        tr = ncu_traffic(args.workload, "k4_span")
         roofline = {
-            "bound": "alu", "kernel": "k4_brick", "achieved": achieved, "peak": peak_alu, "unit": "Tops/s (INT32)",
-            "frac": achieved / peak_alu, "traffic": None,
+            "bound": "alu", "kernel": "k4_span", "achieved": achieved, "peak": peak_alu, "unit": "Tops/s (INT32)",
+            "frac": achieved / peak_alu, "traffic": (tr or {}).get("bytes"), "traffic_source": (tr or {}).get("source"),
             "model": f"{OPS_PER_SAMPLE:g} ops/candidate sample + {OPS_PER_PAIR:g} ops/(tet,tile) pair",
             "ops_per_launch": ops, "kernel_ms": k4,
             "peak_source": "derived: 148 SMs x 64 alu-pipe lanes x clocks.max.sm (DESIGN.md Roofline)",

@@ -179,52 +179,88 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
 }
 
 // ------------------------------------------------------------------------------------------
-// K2: exclusive scan of counts[0..NB) (single CTA; NB is at most a few 10^5)
+// K2: exclusive scan of counts[0..NB) (single CTA, 4096 counters per pass; NB is at most a few 10^5)
 // counts[b] <- offset, counts[NB] <- total, cursor[b] <- offset
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(1024) k2_scan(u32 NB, u32* __restrict__ counts, u32* __restrict__ cursor,
                                                 u32* __restrict__ hdr) {
-    __shared__ u64 s_part[1024];
+    // chunks of 4096 counters: one coalesced uint4 per thread, warp shuffle scan, 32 warp partials
+    // scanned by warp 0, running carry in 64 bits (a total above 2^32 raises the overflow flag)
+    __shared__ u64 s_warp[32];
+    __shared__ u64 s_carry;
     __shared__ u32 s_ne[32];
-    const int tid = threadIdx.x;
-    const u32 per = (NB + 1023u) / 1024u;
-    const u32 beg = min(NB, (u32)tid * per), end = min(NB, beg + per);
-    u64 sum = 0;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool vec_ok = ((size_t)counts & 15) == 0 && ((size_t)cursor & 15) == 0;
+    if (tid == 0) s_carry = 0;
     u32 ne = 0;
-    for (u32 i = beg; i < end; ++i) {
-        u32 c = counts[i];
-        sum += c;
-        ne += (c != 0);
+    auto load4 = [&](u32 i) {
+        uint4 c = make_uint4(0u, 0u, 0u, 0u);
+        if (i + 3 < NB && vec_ok) c = *reinterpret_cast<const uint4*>(counts + i);
+        else {
+            if (i < NB) c.x = counts[i];
+            if (i + 1 < NB) c.y = counts[i + 1];
+            if (i + 2 < NB) c.z = counts[i + 2];
+            if (i + 3 < NB) c.w = counts[i + 3];
+        }
+        return c;
+    };
+    uint4 nxt = load4((u32)tid * 4u);
+    for (u32 base = 0; base < NB; base += 4096u) {
+        const u32 i = base + (u32)tid * 4u;
+        const uint4 c = nxt;
+        if (base + 4096u < NB) nxt = load4(i + 4096u);  // prefetch the next chunk
+        ne += (c.x != 0) + (c.y != 0) + (c.z != 0) + (c.w != 0);
+        const u64 mine = (u64)c.x + c.y + c.z + c.w;
+        u64 incl = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const u64 v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        __syncthreads();  // s_warp / s_carry of the previous chunk are consumed
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            const u64 w = s_warp[lane];
+            u64 wi = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const u64 v = __shfl_up_sync(0xFFFFFFFFu, wi, o);
+                if (lane >= o) wi += v;
+            }
+            const u64 carry = s_carry;
+            s_warp[lane] = carry + wi - w;  // exclusive offset of each warp, carry included
+            __syncwarp();
+            if (lane == 31) s_carry = carry + wi;
+        }
+        __syncthreads();
+        const u64 run = s_warp[warp] + incl - mine;
+        uint4 o4;
+        o4.x = (u32)run;
+        o4.y = (u32)(run + c.x);
+        o4.z = (u32)(run + c.x + c.y);
+        o4.w = (u32)(run + c.x + c.y + c.z);
+        if (i + 3 < NB && vec_ok) {
+            *reinterpret_cast<uint4*>(counts + i) = o4;
+            *reinterpret_cast<uint4*>(cursor + i) = o4;
+        } else {
+            if (i < NB) { counts[i] = o4.x; cursor[i] = o4.x; }
+            if (i + 1 < NB) { counts[i + 1] = o4.y; cursor[i + 1] = o4.y; }
+            if (i + 2 < NB) { counts[i + 2] = o4.z; cursor[i + 2] = o4.z; }
+            if (i + 3 < NB) { counts[i + 3] = o4.w; cursor[i + 3] = o4.w; }
+        }
     }
-    s_part[tid] = sum;
-    // non-empty tiles: warp reduce then smem
     for (int o = 16; o; o >>= 1) ne += __shfl_xor_sync(0xFFFFFFFFu, ne, o);
-    if ((tid & 31) == 0) s_ne[tid >> 5] = ne;
+    if (lane == 0) s_ne[warp] = ne;
     __syncthreads();
-    // Hillis-Steele inclusive scan over 1024 partials
-    for (int o = 1; o < 1024; o <<= 1) {
-        u64 v = (tid >= o) ? s_part[tid - o] : 0;
-        __syncthreads();
-        s_part[tid] += v;
-        __syncthreads();
-    }
-    u64 run = s_part[tid] - sum;  // exclusive
-    for (u32 i = beg; i < end; ++i) {
-        u32 c = counts[i];
-        counts[i] = (u32)run;
-        cursor[i] = (u32)run;
-        run += c;
-    }
-    if (tid == 1023) {
-        u64 total = s_part[1023];
+    if (tid == 0) {
+        const u64 total = s_carry;
         counts[NB] = (u32)min(total, (u64)0xFFFFFFFFu);
         hdr[H_TOTAL] = (u32)total;
         hdr[H_TOTAL_HI] = (u32)(total >> 32);
         if (total > 0xFFFFFFFFull) hdr[H_OVERFLOW] = 1;
-    }
-    if (tid == 0) {
         u32 s = 0;
-        for (int i = 0; i < 32; ++i) s += s_ne[i];
+        for (int k = 0; k < 32; ++k) s += s_ne[k];
         hdr[H_NONEMPTY] = s;
     }
 }

@@ -75,6 +75,19 @@ def test_parity_small_configs(name):
         assert np.all(got == np.uint32(0xFFFFFFFF))
 
 
+@pytest.mark.parametrize("name", ["cfg3", "cfg4", "cfg5"])
+def test_parity_full_size_configs(name):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (default tile and
+    variant, vox_plan for the workspace): the whole grid against the oracle, which finishes each
+    of these in seconds (3.4e9 candidate samples at cfg4)."""
+    m = meshgen.make_config(name)
+    exp = cpu_voxelize(m)
+    got = gpu_voxelize(m)
+    assert_same(got, exp, name + " full size")
+    if m.expect_all_ones:
+        assert np.all(got == np.uint32(0xFFFFFFFF))
+
+
 @pytest.mark.parametrize("tile", [(32, 32), (8, 8), (16, 4), (4, 32), (32, 4)])
 @pytest.mark.parametrize("name", ["cfg2", "cfg4_small_drop3", "giant128_sphere"])
 def test_parity_is_tile_independent(name, tile):
