@@ -34,6 +34,7 @@ struct Params {
     int batch;
     int nx, ny, nz;
     int hx, hy, hz;      // pitch per axis
+    int qx, qy, qz;      // log2(2h) per axis, or -1 when 2h is not a power of two
     int g, g_shift;      // gcd of the pitches; log2(g) or -1
     int sx, sy, sz;      // h / g
     int ty_log, tz_log;  // tile = 32 x (1<<ty_log) x (1<<tz_log) voxels
@@ -89,6 +90,10 @@ __device__ __forceinline__ int floor_div_i(int a, int b) {  // b > 0
     int r = a - q * b;
     return (r < 0) ? q - 1 : q;
 }
+// floor(a / 2h): an arithmetic shift when 2h is a power of two (sh = log2(2h)), else a division
+__device__ __forceinline__ int floor_div_2h(int a, int h, int sh) {
+    return (sh >= 0) ? (a >> sh) : floor_div_i(a, 2 * h);
+}
 __device__ __forceinline__ i64 floor_div_l(i64 a, i64 b) {  // b > 0
     i64 q = a / b;
     i64 r = a - q * b;
@@ -119,11 +124,11 @@ __device__ __forceinline__ i64 six_volume(const Tet& q) {
 }
 
 // closed voxel-index range of centres h*i + h/2 inside [lo, hi], clamped to the grid
-__device__ __forceinline__ void axis_range(int a, int b, int c, int d, int h, int n, int& i0, int& i1) {
+__device__ __forceinline__ void axis_range(int a, int b, int c, int d, int h, int sh, int n, int& i0, int& i1) {
     int lo = min(min(a, b), min(c, d));
     int hi = max(max(a, b), max(c, d));
-    i0 = -floor_div_i(h - 2 * lo, 2 * h);  // ceil((2lo - h) / 2h)
-    i1 = floor_div_i(2 * hi - h, 2 * h);
+    i0 = -floor_div_2h(h - 2 * lo, h, sh);  // ceil((2lo - h) / 2h)
+    i1 = floor_div_2h(2 * hi - h, h, sh);
     i0 = max(i0, 0);
     i1 = min(i1, n - 1);
 }
@@ -153,9 +158,9 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
     if (t < p.T) {
         Tet q = load_tet(p, t);
         int x0, x1, y0, y1, z0, z1;
-        axis_range(q.ax, q.bx, q.cx, q.dx, p.hx, p.nx, x0, x1);
-        axis_range(q.ay, q.by, q.cy, q.dy, p.hy, p.ny, y0, y1);
-        axis_range(q.az, q.bz, q.cz, q.dz, p.hz, p.nz, z0, z1);
+        axis_range(q.ax, q.bx, q.cx, q.dx, p.hx, p.qx, p.nx, x0, x1);
+        axis_range(q.ay, q.by, q.cy, q.dy, p.hy, p.qy, p.ny, y0, y1);
+        axis_range(q.az, q.bz, q.cz, q.dz, p.hz, p.qz, p.nz, z0, z1);
         live = (x0 <= x1) && (y0 <= y1) && (z0 <= z1) && (six_volume(q) != 0);
         if (live) {
             b0x = x0 >> 5; b1x = x1 >> 5;
@@ -169,12 +174,25 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
     }
     unsigned dead = __ballot_sync(0xFFFFFFFFu, (t < p.T) && !live);
     if ((threadIdx.x & 31) == 0 && dead) atomicAdd(hdr + H_CULLED, __popc(dead));
-    if (live) {
-        for (int bz = b0z; bz <= b1z; ++bz)
-            for (int by = b0y; by <= b1y; ++by) {
-                u32 base = (((u32)m * p.nbz + bz) * p.nby + by) * p.nbx;
-                for (int bx = b0x; bx <= b1x; ++bx) atomicAdd(counts + base + bx, 1u);
+    // warp-aggregated histogram: in step k every live lane names the k-th tile of its range; lanes
+    // naming the same tile (neighbouring tets mostly do) are merged into one atomic
+    int cx = b0x, cy = b0y, cz = b0z;
+    const int lane = threadIdx.x & 31;
+    for (;;) {
+        const unsigned act = __ballot_sync(0xFFFFFFFFu, live);
+        if (!act) break;
+        if (live) {
+            const u32 b = ((((u32)m * p.nbz + cz) * p.nby + cy) * p.nbx) + cx;
+            const unsigned peers = __match_any_sync(act, b);
+            if (lane == __ffs(peers) - 1) atomicAdd(counts + b, (u32)__popc(peers));
+            if (++cx > b1x) {
+                cx = b0x;
+                if (++cy > b1y) {
+                    cy = b0y;
+                    live = (++cz <= b1z);
+                }
             }
+        }
     }
 }
 
@@ -271,21 +289,43 @@ __global__ void __launch_bounds__(1024) k2_scan(u32 NB, u32* __restrict__ counts
 __global__ void __launch_bounds__(256) k3_scatter(Params p, const uint2* __restrict__ range, u32* __restrict__ cursor,
                                                   u32* __restrict__ list, u32* __restrict__ hdr) {
     i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= p.T) return;
-    uint2 r = range[t];
-    if (r.x == RANGE_CULLED) return;
-    int b0x = r.x & 1023, b0y = (r.x >> 10) & 1023, b0z = (r.x >> 20) & 1023;
-    int b1x = r.y & 1023, b1y = (r.y >> 10) & 1023, b1z = (r.y >> 20) & 1023;
-    int m = mesh_of(p, t);
-    for (int bz = b0z; bz <= b1z; ++bz)
-        for (int by = b0y; by <= b1y; ++by) {
-            u32 base = (((u32)m * p.nbz + bz) * p.nby + by) * p.nbx;
-            for (int bx = b0x; bx <= b1x; ++bx) {
-                u32 pos = atomicAdd(cursor + base + bx, 1u);
-                if (pos < p.cap) list[pos] = (u32)t;
-                else hdr[H_OVERFLOW] = 1;
+    bool live = false;
+    int b0x = 0, b0y = 0, b1x = 0, b1y = 0, b1z = 0, cx = 0, cy = 0, cz = 0, m = 0;
+    if (t < p.T) {
+        const uint2 r = range[t];
+        if (r.x != RANGE_CULLED) {
+            live = true;
+            b0x = r.x & 1023; b0y = (r.x >> 10) & 1023; cz = (r.x >> 20) & 1023;
+            b1x = r.y & 1023; b1y = (r.y >> 10) & 1023; b1z = (r.y >> 20) & 1023;
+            cx = b0x; cy = b0y;
+            m = mesh_of(p, t);
+        }
+    }
+    // warp-aggregated cursor bump (same stepping as K1): one atomic per distinct tile per step,
+    // the lanes of a group take consecutive slots (order inside a tile list is irrelevant: OR)
+    const int lane = threadIdx.x & 31;
+    for (;;) {
+        const unsigned act = __ballot_sync(0xFFFFFFFFu, live);
+        if (!act) break;
+        if (live) {
+            const u32 b = ((((u32)m * p.nbz + cz) * p.nby + cy) * p.nbx) + cx;
+            const unsigned peers = __match_any_sync(act, b);
+            const int leader = __ffs(peers) - 1;
+            u32 base = 0;
+            if (lane == leader) base = atomicAdd(cursor + b, (u32)__popc(peers));
+            base = __shfl_sync(peers, base, leader);
+            const u32 pos = base + (u32)__popc(peers & ((1u << lane) - 1u));
+            if (pos < p.cap) list[pos] = (u32)t;
+            else hdr[H_OVERFLOW] = 1;
+            if (++cx > b1x) {
+                cx = b0x;
+                if (++cy > b1y) {
+                    cy = b0y;
+                    live = (++cz <= b1z);
+                }
             }
         }
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -351,9 +391,9 @@ __device__ __forceinline__ u32 pack_box(int x0, int x1, int y0, int y1, int z0, 
 // local (tile-relative) closed box of the tet's voxel bbox, intersected with the tile
 __device__ __forceinline__ u32 local_box(const Params& p, const Tet& q, int X0, int Y0, int Z0) {
     int x0, x1, y0, y1, z0, z1;
-    axis_range(q.ax, q.bx, q.cx, q.dx, p.hx, p.nx, x0, x1);
-    axis_range(q.ay, q.by, q.cy, q.dy, p.hy, p.ny, y0, y1);
-    axis_range(q.az, q.bz, q.cz, q.dz, p.hz, p.nz, z0, z1);
+    axis_range(q.ax, q.bx, q.cx, q.dx, p.hx, p.qx, p.nx, x0, x1);
+    axis_range(q.ay, q.by, q.cy, q.dy, p.hy, p.qy, p.ny, y0, y1);
+    axis_range(q.az, q.bz, q.cz, q.dz, p.hz, p.qz, p.nz, z0, z1);
     const int TY = 1 << p.ty_log, TZ = 1 << p.tz_log;
     x0 = max(x0 - X0, 0); x1 = min(x1 - X0, 31);
     y0 = max(y0 - Y0, 0); y1 = min(y1 - Y0, TY - 1);
@@ -526,14 +566,14 @@ __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__
 //   hi-type (mx_G < 0): Q = G                     -> x <= b,  b = max{x : G(x) >= 0}
 //   lo-type (mx_G > 0): Q = -G - 1  (G <= -1)     -> x <= b  <=> G(x) < 0, so the half-space is x >= b+1
 //   mx_G == 0:          Q = 64*G + 63 - x (hi)    -> equivalent on x in [0,63] for integer G
-// b = floor of the real crossing.  A float PROPOSES c0 = rint(Q_row * (1/|mx|)), clamped to [-1,32];
-// the INTEGER value Q(c0) decides: b = c0 if Q(c0) >= 0 else c0-1.  The proposal is within 0.5 of the
-// crossing whenever that lies in [-1.5,32.5] (relative float error <= 2^-21), so b is exact there, and
-// saturates correctly outside.  All Q(x), x in [-1,32], fit int32 (checked in int64 at setup).
+// b = floor of the real crossing r/|mx|.  A fixed-point reciprocal PROPOSES c0 = floor(r*inv/2^32), which is
+// B or B+1 for r >= 0 (see span_bound); the INTEGER value Q(c0) decides: b = c0 if Q(c0) >= 0 else c0-1.
+// No floating point at all.  Planes are stored scaled by 2 (by 4 when |mx| = 1) so that |mx| >= 4 and the
+// reciprocal fits int32; all stored Q(x), x in [-1,32], and r +- mx fit int32 (checked in int64 at setup).
 // ------------------------------------------------------------------------------------------
 enum { SREC_W = 36, KIND_SPAN = 0, IMG_SKEW = 11 };  // record stride 36 words: int4-aligned
-// record words: [0..3] mx  [4..7] my  [8..11] mz  [12..15] g0 (at row y0,z0)  [16..19] 1/|mx| (float bits)
-//               [20] x0-1  [21] x1  [22] ny  [23] nrows  [24] image index of row (y0,z0)
+// record words: [0..3] mx  [4..7] my  [8..11] mz  [12..15] g0 (at row y0,z0)  [16..19] ceil(2^32/|mx|)
+//               [20] x0-1  [21] x1  [22] ny  [23] nrows  [24] shared byte address of image row (y0,z0)
 //               [25] div magic  [26] nlo | kind<<8  [27] tet id  [28] packed local box
 // image: row (y,z) of the tile lives at img[z*(TY+IMG_SKEW) + y] (skew spreads a tet's rows over banks)
 
@@ -550,13 +590,17 @@ __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, i
         ok = (iabs64(g0) < (1ll << 40));
         mx = -1; my *= 64; mz *= 64; g0 = g0 * 64 + 63;
     }
-    const i64 bound = iabs64(g0) + 130 * iabs64(mx) + 32 * (iabs64(my) + iabs64(mz));
+    // stored plane = S*Q with S*|mx| >= 4, so that the reciprocal ceil(2^32 / (S*|mx|)) fits int32
+    const int sh = (mx == -1) ? 2 : 1;
+    mx <<= sh; my <<= sh; mz <<= sh; g0 <<= sh;
+    const i64 bound = iabs64(g0) + 34 * iabs64(mx) + 32 * (iabs64(my) + iabs64(mz));
     ok = ok && (bound < 0x7FFFFF00ll);
+    const u32 a = (u32)(-mx);
     rec[pos] = (int)mx;
     rec[4 + pos] = (int)my;
     rec[8 + pos] = (int)mz;
     rec[12 + pos] = (int)(g0 + my * y0 + mz * z0);
-    rec[16 + pos] = __float_as_int(1.0f / (float)(-(int)mx));
+    rec[16 + pos] = (int)((0xFFFFFFFFu / a) + 1u);  // >= 2^32/a, < 2^32/a + 1; a >= 4 -> < 2^31
     return ok;
 }
 
@@ -564,16 +608,16 @@ __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, i
 // axis (all edge components < 2^15, so every cross-product component is < 2^31) and g a power of two;
 // anything else, or plane values that do not fit int32 on the tile, is handed to the int64 large path.
 __device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0, int Y0, int Z0, int img_stride,
-                                                  int* rec) {
+                                                  u32 img_saddr, int* rec) {
     const Tet q = load_tet(p, t);
     const int lox = min(min(q.ax, q.bx), min(q.cx, q.dx)), hix = max(max(q.ax, q.bx), max(q.cx, q.dx));
     const int loy = min(min(q.ay, q.by), min(q.cy, q.dy)), hiy = max(max(q.ay, q.by), max(q.cy, q.dy));
     const int loz = min(min(q.az, q.bz), min(q.cz, q.dz)), hiz = max(max(q.az, q.bz), max(q.cz, q.dz));
     // local closed voxel box (same rounding as K1's axis_range), clipped to the tile
     const int TY = 1 << p.ty_log, TZ = 1 << p.tz_log;
-    int x0 = -floor_div_i(p.hx - 2 * lox, 2 * p.hx), x1 = floor_div_i(2 * hix - p.hx, 2 * p.hx);
-    int y0 = -floor_div_i(p.hy - 2 * loy, 2 * p.hy), y1 = floor_div_i(2 * hiy - p.hy, 2 * p.hy);
-    int z0 = -floor_div_i(p.hz - 2 * loz, 2 * p.hz), z1 = floor_div_i(2 * hiz - p.hz, 2 * p.hz);
+    int x0 = -floor_div_2h(p.hx - 2 * lox, p.hx, p.qx), x1 = floor_div_2h(2 * hix - p.hx, p.hx, p.qx);
+    int y0 = -floor_div_2h(p.hy - 2 * loy, p.hy, p.qy), y1 = floor_div_2h(2 * hiy - p.hy, p.hy, p.qy);
+    int z0 = -floor_div_2h(p.hz - 2 * loz, p.hz, p.qz), z1 = floor_div_2h(2 * hiz - p.hz, p.hz, p.qz);
     x0 = max(x0 - X0, 0); x1 = min(min(x1, p.nx - 1) - X0, 31);
     y0 = max(y0 - Y0, 0); y1 = min(min(y1, p.ny - 1) - Y0, TY - 1);
     z0 = max(z0 - Z0, 0); z1 = min(min(z1, p.nz - 1) - Z0, TZ - 1);
@@ -612,7 +656,7 @@ __device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0
     a.x = x0 - 1; a.y = x1; a.z = ny; a.w = nrows;
     *reinterpret_cast<int4*>(rec + 20) = a;
     int4 b;
-    b.x = z0 * img_stride + y0;
+    b.x = (int)(img_saddr + 4u * (u32)(z0 * img_stride + y0));
     b.y = (int)((65536u + ny - 1) / ny);
     b.z = nlo | ((ok ? KIND_SPAN : KIND_LARGE) << 8);
     b.w = (int)t;
@@ -620,25 +664,29 @@ __device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0
     rec[28] = (int)pack_box(x0, x1, y0, y1, z0, z1);
 }
 
-// b = max{x in [-128,127] : Q(x) >= 0} (one less if none), Q(x) = r + mx*x, mx < 0.
-// F2I.S8 saturates, which bounds |mx*c0| (the int32 fit check at setup covers |x| <= 130).
-__device__ __forceinline__ int span_bound(int r, int mx, float inv) {
-    const float xf = __int2float_rn(r) * inv;
-    int c0;
-    asm("cvt.rni.s8.f32 %0, %1;" : "=r"(c0) : "f"(xf));
+// b = max{x : Q(x) >= 0} for Q(x) = r + mx*x, mx < 0, whenever r >= 0; some b <= -1 when r < 0.
+// c0 = floor(r * inv / 2^32) with inv in [2^32/|mx|, 2^32/|mx| + 1) and |r| < 2^31 lies in
+// {B, B+1} (B = floor(r/|mx|)) for r >= 0 and is <= -1 for r < 0; the INTEGER value Q(c0) decides.
+// |mx*c0| <= |r| + |mx| < 2^31 (checked at setup), so nothing wraps.
+__device__ __forceinline__ int span_bound(int r, int mx, int inv) {
+    const int c0 = __mulhi(r, inv);
     const int v = r + mx * c0;
     return c0 + (v >> 31);
 }
 
+__device__ __forceinline__ void smem_or(u32 saddr, u32 v) {
+    asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
+}
+
 template <int NLO>
-__device__ __forceinline__ void raster_span(const int* rec, u32* img, int lane, int img_stride) {
+__device__ __forceinline__ void raster_span(const int* rec, int lane, int img_stride) {
     const int4 MX = *reinterpret_cast<const int4*>(rec);
     const int4 MY = *reinterpret_cast<const int4*>(rec + 4);
     const int4 MZ = *reinterpret_cast<const int4*>(rec + 8);
     const int4 G0 = *reinterpret_cast<const int4*>(rec + 12);
-    const float4 IV = *reinterpret_cast<const float4*>(rec + 16);
+    const int4 IV = *reinterpret_cast<const int4*>(rec + 16);
     const int4 A = *reinterpret_cast<const int4*>(rec + 20);  // x0-1, x1, ny, nrows
-    const int2 B = *reinterpret_cast<const int2*>(rec + 24);  // image index of row (y0,z0), div magic
+    const int2 B = *reinterpret_cast<const int2*>(rec + 24);  // shared byte address of row (y0,z0), div magic
     for (int r = lane; r < A.w; r += 32) {
         const int zz = (int)(((u32)r * (u32)B.y) >> 16);
         const int yy = r - zz * A.z;
@@ -653,7 +701,7 @@ __device__ __forceinline__ void raster_span(const int* rec, u32* img, int lane, 
         const int n = upper - lower;  // number of solid voxels in the row
         if (n > 0) {
             const u32 word = (0xFFFFFFFFu >> (32 - n)) << (lower + 1);
-            atomicOr(img + B.x + zz * img_stride + yy, word);
+            smem_or((u32)B.x + 4u * (u32)(zz * img_stride + yy), word);
         }
     }
 }
@@ -677,22 +725,23 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
     const int X0 = bx << 5, Y0 = by << p.ty_log, Z0 = bz << p.tz_log;
     const int TY = 1 << p.ty_log, img_stride = TY + IMG_SKEW;
     const int img_words = img_stride << p.tz_log;
+    const u32 img_saddr = (u32)__cvta_generic_to_shared(img);
     for (int i = tid; i < img_words; i += NT) img[i] = 0;
     if (tid == 0) s_large = 0;
     const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
     for (u32 base = beg; base < end; base += NT) {
         __syncthreads();
         const int n = min((u32)NT, end - base);
-        if (tid < n) setup_span_record(p, list[base + tid], X0, Y0, Z0, img_stride, rec[tid]);
+        if (tid < n) setup_span_record(p, list[base + tid], X0, Y0, Z0, img_stride, img_saddr, rec[tid]);
         __syncthreads();
         for (int i = warp; i < n; i += NW) {
             const int* r = rec[i];
             const int info = r[26];
             if ((info >> 8) == KIND_SPAN) {
                 const int nlo = info & 255;
-                if (nlo == 2) raster_span<2>(r, img, lane, img_stride);
-                else if (nlo == 1) raster_span<1>(r, img, lane, img_stride);
-                else if (nlo == 3) raster_span<3>(r, img, lane, img_stride);
+                if (nlo == 2) raster_span<2>(r, lane, img_stride);
+                else if (nlo == 1) raster_span<1>(r, lane, img_stride);
+                else if (nlo == 3) raster_span<3>(r, lane, img_stride);
                 // nlo == 0 or 4 cannot happen for a non-degenerate tet (the four sigma*N sum to zero
                 // and planes with N_x == 0 count as hi-type): nothing to draw
             } else {
@@ -820,6 +869,7 @@ extern "C" int vox_create(vox_ctx** out, int nx, int ny, int nz, int ex, int ey,
     Params& p = c->p;
     p.nx = nx; p.ny = ny; p.nz = nz; p.ex = ex; p.ey = ey; p.ez = ez; p.batch = batch;
     p.hx = ex / nx; p.hy = ey / ny; p.hz = ez / nz;
+    p.qx = ilog2_exact(2 * p.hx); p.qy = ilog2_exact(2 * p.hy); p.qz = ilog2_exact(2 * p.hz);
     p.g = gcd_i(gcd_i(p.hx, p.hy), p.hz);
     p.g_shift = ilog2_exact(p.g);
     p.sx = p.hx / p.g; p.sy = p.hy / p.g; p.sz = p.hz / p.g;
