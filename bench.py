@@ -45,7 +45,8 @@ def _args():
     ap.add_argument("--workload", default="cfg4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--e2e-steps", type=int, default=20)
+    ap.add_argument("--e2e-depth", type=int, default=3)
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--tile", type=int, nargs=2, default=None)
     return ap.parse_args()
@@ -327,38 +328,59 @@ def run_b200(args):
         sec = tmax * 1e-3
         value = ssum * args.steps / sec / 1e9
 
-        # ---- e2e: HOST buffers through vox_run_host (H2D of the mesh, run, D2H of the grid)
+        # ---- e2e: HOST buffers in, HOST grid out, through the public vox_pipe_* calls.  Every step
+        # copies that step's mesh from pinned host memory (H2D), runs the hot path and copies the
+        # grid back (D2H); `depth` meshes are in flight so step k's copies overlap step k+-1's
+        # kernels.  Also reported: the unpipelined vox_run_host call (one mesh, fully serialised).
         e2e = None
         if not args.no_e2e:
             hv = torch.from_numpy(m.verts).pin_memory()
             ht = torch.from_numpy(m.tets).pin_memory()
             ho = torch.from_numpy(off_np).pin_memory() if off_np is not None else None
-            hout = torch.empty((m.batch, nz, ny, nx // 32), dtype=torch.int32).pin_memory()
-            vz2 = pkg.Voxelizer(m.grid, m.extent, m.batch, tile=args.tile, variant=args.variant)
-            need = vz2.host_arena_bytes(m.V, m.T)
-            arena = torch.empty(need, dtype=torch.uint8, device="cuda")
-            for _ in range(2):
-                vz2.run_host(hv, ht, hout, arena, ho, stream)
+            depth = args.e2e_depth
+            houts = [torch.empty((m.batch, nz, ny, nx // 32), dtype=torch.int32).pin_memory() for _ in range(depth)]
+            pipe = pkg.Pipe(m.grid, m.extent, m.batch, depth=depth, max_V=m.V, max_T=m.T, tile=args.tile,
+                            variant=args.variant)
+
+            def pipe_steps(k):
+                tickets = []
+                for i in range(k):
+                    if i >= depth:
+                        pipe.wait(tickets[i - depth])
+                    tickets.append(pipe.submit(hv, ht, houts[i % depth], ho))
+                for t in tickets[max(0, k - depth):]:
+                    pipe.wait(t)
+
+            pipe_steps(max(3, depth))  # warm-up
             barrier()
             torch.cuda.synchronize()
             t0 = time.perf_counter()
-            f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            f0.record(stream)
-            for _ in range(args.e2e_steps):
-                vz2.run_host(hv, ht, hout, arena, ho, stream)  # synchronises each step
-            f1.record(stream)
+            pipe_steps(args.e2e_steps)
             torch.cuda.synchronize()
-            wall = time.perf_counter() - t0
-            e2e_ms = max(f0.elapsed_time(f1), wall * 1e3)
+            e2e_ms = (time.perf_counter() - t0) * 1e3  # host wall clock around submit..wait of all steps
             e2e_ms = reduce_over_ranks(dist, e2e_ms, 0, 0, "cuda")[0]
-            h2d = hv.numel() * 4 + ht.numel() * 4 + (ho.numel() * 8 if ho is not None else 0)
-            d2h = hout.numel() * 4 + 256  # grid + the status header
-            e2e = {"value": ssum * args.e2e_steps / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
-                   "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.e2e_steps,
-                   "steps": args.e2e_steps,
-                   "same_result": bool(rank != 0 or torch.equal(hout, out.cpu()))}
+            same = bool(rank != 0 or all(torch.equal(h, out.cpu()) for h in houts[:min(depth, args.e2e_steps)]))
+            pipe.close()
+            # unpipelined single call
+            vz2 = pkg.Voxelizer(m.grid, m.extent, m.batch, tile=args.tile, variant=args.variant)
+            arena = torch.empty(vz2.host_arena_bytes(m.V, m.T), dtype=torch.uint8, device="cuda")
+            for _ in range(2):
+                vz2.run_host(hv, ht, houts[0], arena, ho, stream)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(3):
+                vz2.run_host(hv, ht, houts[0], arena, ho, stream)  # synchronises each call
+            sync_ms = (time.perf_counter() - t0) * 1e3 / 3
             vz2.close()
             del arena
+            h2d = hv.numel() * 4 + ht.numel() * 4 + (ho.numel() * 8 if ho is not None else 0)
+            d2h = houts[0].numel() * 4 + 256  # grid + the status header
+            e2e = {"value": ssum * args.e2e_steps / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
+                   "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.e2e_steps,
+                   "steps": args.e2e_steps, "api": f"vox_pipe_submit/vox_pipe_wait, depth {depth}",
+                   "same_result": same,
+                   "unpipelined_vox_run_host": {"ms_per_call": sync_ms,
+                                                "value": float(samples) / (sync_ms * 1e-3) / 1e9}}
 
         if rank != 0:
             vz.close()
@@ -418,7 +440,7 @@ def run_b200(args):
             "mtets_per_s": tsum * args.steps / sec / 1e6,
             "gvoxels_per_s": world * m.batch * nx * ny * nz * args.steps / sec / 1e9,
             "kernel_ms": shares, "status": st, "popcount": popcount,
-            "gpu_launches": args.steps * 4 + (args.e2e_steps * 4 if e2e else 0),
+            "gpu_launches": 4 * (args.steps + ((args.e2e_steps + max(3, args.e2e_depth) + 5) if e2e else 0)),
             "clocks": clk.summary(), "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
         }
         line["config"].pop("tile")

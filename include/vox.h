@@ -119,6 +119,45 @@ int vox_run_host(vox_ctx* ctx, void* cuda_stream, const int32_t* h_verts, int64_
                  const int32_t* h_tets, int64_t T, const int64_t* h_tet_offsets,
                  void* d_arena, size_t arena_bytes, uint32_t* h_bits_out);
 
+/* Transfer-overlapped pipeline for a STREAM of meshes in host memory.
+ * The paper's own tables say the host<->device copies, not the kernel, dominate
+ * ("the overhead of copying data to GPU memory"; Table 2),
+ * so consecutive meshes are overlapped: while mesh k is voxelized, mesh k+1 is copied in
+ * and grid k-1 is copied out, on three internal non-blocking streams, `depth` meshes in
+ * flight.  Every mesh runs exactly the vox_tets + vox_run path above.
+ *
+ *   vox_pipe_create   grid/extent/batch as vox_create; depth in [1,8]; max_V/max_T bound
+ *                     the meshes that will be submitted.  Creates streams, events and a
+ *                     small pinned status block per slot (host-side allocations: call it
+ *                     outside any timed region).
+ *   vox_pipe_arena_bytes  device bytes the caller must provide (depth x [verts, tets,
+ *                     offsets, grid, estimated-pairs workspace]).
+ *   vox_pipe_bind     hand over the caller's device arena (borrowed until destroy).
+ *   vox_pipe_submit   enqueue one mesh: H2D of h_verts int32[V][3], h_tets int32[T][4],
+ *                     h_tet_offsets int64[batch+1] (NULL if batch == 1), the hot path,
+ *                     D2H of the grid into h_bits_out (uint32[vox_grid_words]).  Host
+ *                     buffers must be pinned and stay untouched until the ticket is
+ *                     waited on.  Blocks only when all `depth` slots are in flight (then
+ *                     it waits for the oldest).  *ticket_out = 0,1,2,... in submit order.
+ *   vox_pipe_wait     block until that mesh's grid is in h_bits_out; VOX_EWORKSPACE if
+ *                     pairs were dropped (arena workspace too small for this mesh);
+ *                     stats_out as vox_status (may be NULL).  Tickets may be waited once,
+ *                     in any order, but no later than `depth` submits after their own.
+ *   vox_pipe_set_variant / vox_pipe_set_tile   as the vox_ctx calls, for every slot.
+ */
+typedef struct vox_pipe vox_pipe;
+int vox_pipe_create(vox_pipe** out, int nx, int ny, int nz, int ex, int ey, int ez, int batch, int depth,
+                    int64_t max_V, int64_t max_T);
+void vox_pipe_destroy(vox_pipe* pipe);
+int vox_pipe_set_variant(vox_pipe* pipe, int variant);
+int vox_pipe_set_tile(vox_pipe* pipe, int ty, int tz);
+size_t vox_pipe_arena_bytes(const vox_pipe* pipe);
+int vox_pipe_bind(vox_pipe* pipe, void* d_arena, size_t arena_bytes);
+int vox_pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,
+                    const int64_t* h_tet_offsets, uint32_t* h_bits_out, int64_t* ticket_out);
+int vox_pipe_wait(vox_pipe* pipe, int64_t ticket, int64_t stats_out[4]);
+const char* vox_pipe_last_error(const vox_pipe* pipe);
+
 /* Benchmark instrumentation (off by default).  vox_timing_enable(ctx, slots > 0)
  * creates a ring of CUDA events (a host-side allocation: call it outside any timed
  * region); every later vox_run then records an event on its stream before K1's

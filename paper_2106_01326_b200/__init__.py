@@ -7,6 +7,7 @@ that the build can be checked), but every compute call needs the library and a
 CUDA device and fails loudly otherwise.
 """
 from .binding import (  # noqa: F401
+    Pipe,
     VoxError,
     Voxelizer,
     lib_path,

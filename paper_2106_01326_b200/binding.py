@@ -14,6 +14,8 @@ EXPORTS = [
     "vox_workspace_bytes", "vox_workspace_fixed_bytes", "vox_plan", "vox_run", "vox_status",
     "vox_validate", "vox_host_arena_bytes", "vox_run_host", "vox_timing_enable", "vox_timing_read",
     "vox_probe_int32", "vox_strerror", "vox_last_error",
+    "vox_pipe_create", "vox_pipe_destroy", "vox_pipe_set_variant", "vox_pipe_set_tile", "vox_pipe_arena_bytes",
+    "vox_pipe_bind", "vox_pipe_submit", "vox_pipe_wait", "vox_pipe_last_error",
 ]
 
 
@@ -59,6 +61,15 @@ def load_library():
         "vox_probe_int32": (i32, [vp, i32, i32, i32, vp, ctypes.POINTER(ctypes.c_double)]),
         "vox_strerror": (ctypes.c_char_p, [i32]),
         "vox_last_error": (ctypes.c_char_p, [vp]),
+        "vox_pipe_create": (i32, [ctypes.POINTER(vp), i32, i32, i32, i32, i32, i32, i32, i32, i64, i64]),
+        "vox_pipe_destroy": (None, [vp]),
+        "vox_pipe_set_variant": (i32, [vp, i32]),
+        "vox_pipe_set_tile": (i32, [vp, i32, i32]),
+        "vox_pipe_arena_bytes": (sz, [vp]),
+        "vox_pipe_bind": (i32, [vp, vp, sz]),
+        "vox_pipe_submit": (i32, [vp, vp, i64, vp, i64, vp, vp, ctypes.POINTER(i64)]),
+        "vox_pipe_wait": (i32, [vp, i64, ctypes.POINTER(i64)]),
+        "vox_pipe_last_error": (ctypes.c_char_p, [vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -241,6 +252,73 @@ class Voxelizer:
             "vox_run_host",
         )
         return h_out
+
+
+class Pipe:
+    """vox_pipe_*: transfer-overlapped voxelization of a stream of meshes held in pinned host memory.
+
+    submit() takes pinned CPU tensors (verts int32[V][3], tets int32[T][4], optional offsets
+    int64[batch+1]) and a pinned CPU output tensor int32[batch][nz][ny][nx/32]; wait(ticket)
+    blocks until that output is complete and returns the run's statistics."""
+
+    def __init__(self, grid, extent=(65536, 65536, 65536), batch=1, depth=3, max_V=0, max_T=0, tile=None, variant=0):
+        torch = _torch_cuda()
+        self._lib = load_library()
+        self._p = ctypes.c_void_p()
+        self.grid = tuple(int(g) for g in grid)
+        self.batch, self.depth = int(batch), int(depth)
+        rc = self._lib.vox_pipe_create(ctypes.byref(self._p), *self.grid, *(int(e) for e in extent), self.batch,
+                                       self.depth, int(max_V), int(max_T))
+        if rc:
+            raise VoxError(rc, "vox_pipe_create")
+        if tile is not None:
+            self._ck(self._lib.vox_pipe_set_tile(self._p, int(tile[0]), int(tile[1])), "vox_pipe_set_tile")
+        if variant:
+            self._ck(self._lib.vox_pipe_set_variant(self._p, int(variant)), "vox_pipe_set_variant")
+        self.arena_bytes = int(self._lib.vox_pipe_arena_bytes(self._p))
+        self._arena = torch.empty(self.arena_bytes + 256, dtype=torch.uint8, device="cuda")
+        base = self._arena.data_ptr()
+        self._ck(self._lib.vox_pipe_bind(self._p, ctypes.c_void_p((base + 255) & ~255), self.arena_bytes),
+                 "vox_pipe_bind")
+        self._keep = {}
+
+    def _ck(self, rc, where):
+        if rc:
+            raise VoxError(rc, where, self._lib.vox_pipe_last_error(self._p).decode())
+
+    def submit(self, h_verts, h_tets, h_out, h_tet_offsets=None):
+        for t in (h_verts, h_tets, h_out) + ((h_tet_offsets,) if h_tet_offsets is not None else ()):
+            assert not t.is_cuda and t.is_contiguous() and (t.numel() == 0 or t.is_pinned()), \
+                "pipe buffers must be pinned CPU tensors"
+        ticket = ctypes.c_int64(-1)
+        off_ptr = ctypes.c_void_p(h_tet_offsets.data_ptr()) if h_tet_offsets is not None else None
+        self._ck(
+            self._lib.vox_pipe_submit(self._p, ctypes.c_void_p(h_verts.data_ptr()), h_verts.numel() // 3,
+                                      ctypes.c_void_p(h_tets.data_ptr()), h_tets.numel() // 4, off_ptr,
+                                      ctypes.c_void_p(h_out.data_ptr()), ctypes.byref(ticket)),
+            "vox_pipe_submit",
+        )
+        self._keep[ticket.value] = (h_verts, h_tets, h_out, h_tet_offsets)
+        return int(ticket.value)
+
+    def wait(self, ticket):
+        st = (ctypes.c_int64 * 4)()
+        rc = self._lib.vox_pipe_wait(self._p, int(ticket), st)
+        self._keep.pop(int(ticket), None)
+        self._ck(rc, "vox_pipe_wait")
+        return dict(pairs=int(st[0]), culled=int(st[1]), large_pairs=int(st[2]), nonempty_tiles=int(st[3]))
+
+    def close(self):
+        if self._p:
+            self._lib.vox_pipe_destroy(self._p)
+            self._p = ctypes.c_void_p()
+        self._arena = None
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def voxelize(verts, tets, grid, extent=(65536, 65536, 65536), tet_offsets=None, tile=None, variant=0, exact_plan=True):

@@ -678,7 +678,7 @@ __device__ __forceinline__ void smem_or(u32 saddr, u32 v) {
     asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
 }
 
-template <int NLO>
+template <int NLO, bool UNCOND>
 __device__ __forceinline__ void raster_span(const int* rec, int lane, int img_stride) {
     const int4 MX = *reinterpret_cast<const int4*>(rec);
     const int4 MY = *reinterpret_cast<const int4*>(rec + 4);
@@ -698,15 +698,26 @@ __device__ __forceinline__ void raster_span(const int* rec, int lane, int img_st
         if (NLO == 1) { lower = max(A.x, b0); upper = min(min(A.y, b1), min(b2, b3)); }
         else if (NLO == 2) { lower = max(A.x, max(b0, b1)); upper = min(A.y, min(b2, b3)); }
         else { lower = max(max(A.x, b0), max(b1, b2)); upper = min(A.y, b3); }
-        const int n = upper - lower;  // number of solid voxels in the row
-        if (n > 0) {
-            const u32 word = (0xFFFFFFFFu >> (32 - n)) << (lower + 1);
-            smem_or((u32)B.x + 4u * (u32)(zz * img_stride + yy), word);
+        const int n = upper - lower;  // number of solid voxels in the row (<= 0: none)
+        const u32 saddr = (u32)B.x + 4u * (u32)(zz * img_stride + yy);
+        if (UNCOND) {
+            // branch-free: PTX shifts clamp at 32, so n <= 0 gives word 0 and the OR is a no-op
+            asm volatile(
+                "{\n\t.reg .b32 m, s;\n\t"
+                "sub.s32 s, 32, %1;\n\t"
+                "shr.b32 m, 0xFFFFFFFF, s;\n\t"
+                "add.s32 s, %2, 1;\n\t"
+                "shl.b32 m, m, s;\n\t"
+                "red.shared.or.b32 [%0], m;\n\t}"
+                ::"r"(saddr), "r"(n), "r"(lower)
+                : "memory");
+        } else if (n > 0) {
+            smem_or(saddr, (0xFFFFFFFFu >> (32 - n)) << (lower + 1));
         }
     }
 }
 
-template <int NT, int MINB>
+template <int NT, int MINB, bool UNCOND>
 __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restrict__ offsets,
                                                     const u32* __restrict__ list, u32* __restrict__ bits,
                                                     u32* __restrict__ hdr) {
@@ -729,24 +740,32 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
     for (int i = tid; i < img_words; i += NT) img[i] = 0;
     if (tid == 0) s_large = 0;
     const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
+    u32 seen_large = 0;
     for (u32 base = beg; base < end; base += NT) {
         __syncthreads();
         const int n = min((u32)NT, end - base);
-        if (tid < n) setup_span_record(p, list[base + tid], X0, Y0, Z0, img_stride, img_saddr, rec[tid]);
+        if (tid < n) {
+            setup_span_record(p, list[base + tid], X0, Y0, Z0, img_stride, img_saddr, rec[tid]);
+            if ((rec[tid][26] >> 8) != KIND_SPAN) atomicAdd(&s_large, 1u);
+        }
         __syncthreads();
         for (int i = warp; i < n; i += NW) {
             const int* r = rec[i];
             const int info = r[26];
-            if ((info >> 8) == KIND_SPAN) {
-                const int nlo = info & 255;
-                if (nlo == 2) raster_span<2>(r, lane, img_stride);
-                else if (nlo == 1) raster_span<1>(r, lane, img_stride);
-                else if (nlo == 3) raster_span<3>(r, lane, img_stride);
-                // nlo == 0 or 4 cannot happen for a non-degenerate tet (the four sigma*N sum to zero
-                // and planes with N_x == 0 count as hi-type): nothing to draw
-            } else {
-                raster_large(p, (u32)r[27], (u32)r[28], X0, Y0, Z0, img, lane, img_stride);
-                if (lane == 0) atomicAdd(&s_large, 1u);
+            // nlo == 0 or 4 cannot happen for a non-degenerate tet (the four sigma*N sum to zero
+            // and planes with N_x == 0 count as hi-type); KIND_LARGE (info >= 256) is drawn below
+            if (info == 2) raster_span<2, UNCOND>(r, lane, img_stride);
+            else if (info == 1) raster_span<1, UNCOND>(r, lane, img_stride);
+            else if (info == 3) raster_span<3, UNCOND>(r, lane, img_stride);
+        }
+        // large pairs of this batch (rare): kept out of the loop above so that it holds no call
+        const u32 nl = s_large;  // cumulative; stable between the barrier above and the next one
+        if (nl != seen_large) {
+            seen_large = nl;
+            for (int i = warp; i < n; i += NW) {
+                const int* r = rec[i];
+                if ((r[26] >> 8) != KIND_SPAN)
+                    raster_large(p, (u32)r[27], (u32)r[28], X0, Y0, Z0, img, lane, img_stride);
             }
         }
     }
@@ -1038,10 +1057,14 @@ extern "C" int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_
         k3_scatter<<<blocks, 256, 0, st>>>(p, range, cursor, list, hdr);
     }
     if (ev) CK(cudaEventRecord(ev[3], st));
-    if (ctx->variant == 1) k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
-    else if (ctx->variant == 2) k4_span<256, 2><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
-    else if (ctx->variant == 3) k4_span<256, 4><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr);
-    else k4_span<128, 8><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr);  // 64 regs, 32 warps/SM
+    switch (ctx->variant) {  // A/B variants kept for the parity tests and the sweep in DESIGN.md
+        case 1: k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
+        case 2: k4_span<256, 4, true><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
+        case 4: k4_span<128, 8, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
+        case 5: k4_span<128, 7, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
+        case 6: k4_span<128, 9, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
+        default: k4_span<128, 8, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr);  // 64 regs, 32 warps/SM
+    }
     CK(cudaGetLastError());
     if (ev) {
         CK(cudaEventRecord(ev[4], st));
@@ -1129,6 +1152,194 @@ extern "C" int vox_run_host(vox_ctx* ctx, void* cuda_stream, const int32_t* h_ve
     CK(cudaMemcpyAsync(h_bits_out, a + A.bits, vox_grid_words(ctx) * 4, cudaMemcpyDeviceToHost, st));
     return vox_status(ctx, st, a + A.ws, NULL);
 }
+
+// ------------------------------------------------------------------------------------------
+// vox_pipe: transfer-overlapped pipeline over a stream of host meshes (include/vox.h)
+// ------------------------------------------------------------------------------------------
+enum { PIPE_MAX_DEPTH = 8 };
+struct PipeSlot {
+    vox_ctx* ctx;
+    cudaEvent_t in_done, run_done, out_done;
+    u32* h_hdr;      // pinned, HDR_WORDS
+    i64 ticket;      // ticket in flight in this slot, -1 = free
+    char* base;      // slice of the arena
+};
+struct vox_pipe {
+    int depth;
+    i64 maxV, maxT;
+    i64 next_ticket;
+    cudaStream_t s_in, s_run, s_out;
+    PipeSlot slot[PIPE_MAX_DEPTH];
+    ArenaLayout A;       // layout of one slice (workspace last)
+    size_t slice_bytes;
+    bool bound;
+    char err[256];
+};
+
+static int pipe_fail(vox_pipe* q, cudaError_t e, const char* where) {
+    snprintf(q->err, sizeof(q->err), "%s: %s", where, cudaGetErrorString(e));
+    return VOX_ECUDA;
+}
+#define PCK(call)                                                \
+    do {                                                         \
+        cudaError_t e_ = (call);                                 \
+        if (e_ != cudaSuccess) return pipe_fail(pipe, e_, #call); \
+    } while (0)
+
+static void pipe_layout(vox_pipe* q) {
+    vox_ctx tmp = *q->slot[0].ctx;
+    tmp.p.T = q->maxT;
+    tmp.pairs_planned = -1;
+    q->A = arena_layout(&tmp, q->maxV, q->maxT, vox_workspace_bytes(&tmp));
+    q->slice_bytes = align256(q->A.end);
+}
+
+extern "C" void vox_pipe_destroy(vox_pipe* pipe) {
+    if (!pipe) return;
+    if (pipe->s_out) cudaStreamSynchronize(pipe->s_out);
+    if (pipe->s_run) cudaStreamSynchronize(pipe->s_run);
+    if (pipe->s_in) cudaStreamSynchronize(pipe->s_in);
+    for (int i = 0; i < pipe->depth; ++i) {
+        PipeSlot& s = pipe->slot[i];
+        if (s.in_done) cudaEventDestroy(s.in_done);
+        if (s.run_done) cudaEventDestroy(s.run_done);
+        if (s.out_done) cudaEventDestroy(s.out_done);
+        if (s.h_hdr) cudaFreeHost(s.h_hdr);
+        vox_destroy(s.ctx);
+    }
+    if (pipe->s_in) cudaStreamDestroy(pipe->s_in);
+    if (pipe->s_run) cudaStreamDestroy(pipe->s_run);
+    if (pipe->s_out) cudaStreamDestroy(pipe->s_out);
+    free(pipe);
+}
+
+extern "C" int vox_pipe_create(vox_pipe** out, int nx, int ny, int nz, int ex, int ey, int ez, int batch, int depth,
+                               int64_t max_V, int64_t max_T) {
+    if (!out) return VOX_EINVAL;
+    *out = NULL;
+    if (depth < 1 || depth > PIPE_MAX_DEPTH || max_V < 0 || max_T < 0) return VOX_EINVAL;
+    if (max_T > 0xFFFFFFF0ll || max_V > 0x7FFFFFFFll) return VOX_ERANGE;
+    vox_pipe* pipe = (vox_pipe*)calloc(1, sizeof(vox_pipe));
+    if (!pipe) return VOX_EINVAL;
+    pipe->depth = depth;
+    pipe->maxV = max_V;
+    pipe->maxT = max_T;
+    for (int i = 0; i < depth; ++i) {
+        int rc = vox_create(&pipe->slot[i].ctx, nx, ny, nz, ex, ey, ez, batch);
+        if (rc) { vox_pipe_destroy(pipe); return rc; }
+        pipe->slot[i].ticket = -1;
+    }
+    bool ok = cudaStreamCreateWithFlags(&pipe->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&pipe->s_run, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&pipe->s_out, cudaStreamNonBlocking) == cudaSuccess;
+    for (int i = 0; ok && i < depth; ++i) {
+        PipeSlot& s = pipe->slot[i];
+        ok = cudaEventCreateWithFlags(&s.in_done, cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&s.run_done, cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&s.out_done, cudaEventDisableTiming) == cudaSuccess &&
+             cudaHostAlloc((void**)&s.h_hdr, HDR_WORDS * 4, cudaHostAllocDefault) == cudaSuccess;
+    }
+    if (!ok) { cudaGetLastError(); vox_pipe_destroy(pipe); return VOX_ECUDA; }
+    pipe_layout(pipe);
+    *out = pipe;
+    return VOX_OK;
+}
+
+extern "C" int vox_pipe_set_variant(vox_pipe* pipe, int variant) {
+    if (!pipe) return VOX_EINVAL;
+    for (int i = 0; i < pipe->depth; ++i) vox_set_variant(pipe->slot[i].ctx, variant);
+    return VOX_OK;
+}
+
+extern "C" int vox_pipe_set_tile(vox_pipe* pipe, int ty, int tz) {
+    if (!pipe) return VOX_EINVAL;
+    if (pipe->bound) return VOX_ESTATE;
+    for (int i = 0; i < pipe->depth; ++i) {
+        int rc = vox_set_tile(pipe->slot[i].ctx, ty, tz);
+        if (rc) return rc;
+    }
+    pipe_layout(pipe);
+    return VOX_OK;
+}
+
+extern "C" size_t vox_pipe_arena_bytes(const vox_pipe* pipe) {
+    return pipe ? pipe->slice_bytes * (size_t)pipe->depth : 0;
+}
+
+extern "C" int vox_pipe_bind(vox_pipe* pipe, void* d_arena, size_t arena_bytes) {
+    if (!pipe || !d_arena) return VOX_EINVAL;
+    if (((uintptr_t)d_arena & 255) != 0) return VOX_EINVAL;
+    if (arena_bytes < vox_pipe_arena_bytes(pipe)) return VOX_EWORKSPACE;
+    for (int i = 0; i < pipe->depth; ++i) {
+        if (pipe->slot[i].ticket >= 0) return VOX_ESTATE;
+        pipe->slot[i].base = (char*)d_arena + (size_t)i * pipe->slice_bytes;
+    }
+    pipe->bound = true;
+    return VOX_OK;
+}
+
+static int pipe_finish_slot(vox_pipe* pipe, PipeSlot& s, int64_t stats_out[4]) {
+    PCK(cudaEventSynchronize(s.out_done));
+    s.ticket = -1;
+    const u32* h = s.h_hdr;
+    if (stats_out) {
+        stats_out[0] = (i64)h[H_TOTAL] | ((i64)h[H_TOTAL_HI] << 32);
+        stats_out[1] = h[H_CULLED];
+        stats_out[2] = h[H_LARGE];
+        stats_out[3] = h[H_NONEMPTY];
+    }
+    return h[H_OVERFLOW] ? VOX_EWORKSPACE : VOX_OK;
+}
+
+extern "C" int vox_pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,
+                               const int64_t* h_tet_offsets, uint32_t* h_bits_out, int64_t* ticket_out) {
+    if (!pipe || !h_bits_out || V < 0 || T < 0) return VOX_EINVAL;
+    if (!pipe->bound) return VOX_ESTATE;
+    if (V > pipe->maxV || T > pipe->maxT) return VOX_ERANGE;
+    if (T > 0 && (!h_verts || !h_tets)) return VOX_EINVAL;
+    PipeSlot& s = pipe->slot[pipe->next_ticket % pipe->depth];
+    vox_ctx* ctx = s.ctx;
+    if (ctx->p.batch > 1 && !h_tet_offsets) return VOX_EINVAL;
+    if (s.ticket >= 0) {  // slot still in flight and never waited on: its result is complete but unclaimed
+        PCK(cudaEventSynchronize(s.out_done));
+        s.ticket = -1;
+    }
+    const ArenaLayout& A = pipe->A;
+    char* a = s.base;
+    // copy-in stream
+    if (V > 0) PCK(cudaMemcpyAsync(a + A.verts, h_verts, (size_t)V * 12, cudaMemcpyHostToDevice, pipe->s_in));
+    if (T > 0) PCK(cudaMemcpyAsync(a + A.tets, h_tets, (size_t)T * 16, cudaMemcpyHostToDevice, pipe->s_in));
+    if (ctx->p.batch > 1)
+        PCK(cudaMemcpyAsync(a + A.off, h_tet_offsets, ((size_t)ctx->p.batch + 1) * 8, cudaMemcpyHostToDevice, pipe->s_in));
+    PCK(cudaEventRecord(s.in_done, pipe->s_in));
+    // compute stream
+    PCK(cudaStreamWaitEvent(pipe->s_run, s.in_done, 0));
+    int rc = vox_tets(ctx, (const int32_t*)(a + A.verts), V, (const int32_t*)(a + A.tets), T, (const int64_t*)(a + A.off));
+    if (rc) return rc;
+    rc = vox_run(ctx, pipe->s_run, a + A.ws, pipe->slice_bytes - A.ws, (uint32_t*)(a + A.bits));
+    if (rc) {
+        if (rc == VOX_ECUDA) snprintf(pipe->err, sizeof(pipe->err), "%s", ctx->err);
+        return rc;
+    }
+    PCK(cudaEventRecord(s.run_done, pipe->s_run));
+    // copy-out stream
+    PCK(cudaStreamWaitEvent(pipe->s_out, s.run_done, 0));
+    PCK(cudaMemcpyAsync(h_bits_out, a + A.bits, vox_grid_words(ctx) * 4, cudaMemcpyDeviceToHost, pipe->s_out));
+    PCK(cudaMemcpyAsync(s.h_hdr, a + A.ws + ws_layout(ctx->p).hdr, HDR_WORDS * 4, cudaMemcpyDeviceToHost, pipe->s_out));
+    PCK(cudaEventRecord(s.out_done, pipe->s_out));
+    s.ticket = pipe->next_ticket++;
+    if (ticket_out) *ticket_out = s.ticket;
+    return VOX_OK;
+}
+
+extern "C" int vox_pipe_wait(vox_pipe* pipe, int64_t ticket, int64_t stats_out[4]) {
+    if (!pipe || ticket < 0) return VOX_EINVAL;
+    PipeSlot& s = pipe->slot[ticket % pipe->depth];
+    if (s.ticket != ticket) return VOX_ESTATE;  // never submitted, already waited on, or overwritten
+    return pipe_finish_slot(pipe, s, stats_out);
+}
+
+extern "C" const char* vox_pipe_last_error(const vox_pipe* pipe) { return pipe ? pipe->err : ""; }
 
 extern "C" int vox_probe_int32(void* cuda_stream, int kind, int blocks, int iters, uint32_t* d_sink, double* ops_out) {
     if (blocks <= 0 || iters <= 0 || !d_sink) return VOX_EINVAL;

@@ -259,3 +259,65 @@ def test_validate_flags_bad_data():
     with pytest.raises(pkg.VoxError):
         vz.validate()
     vz.close()
+
+
+# ------------------------------------------------------------------ vox_pipe
+def _pinned(a):
+    import torch
+
+    return torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+
+
+def test_pipe_stream_of_meshes_matches_oracle():
+    """Seven different meshes through a depth-3 pipeline (slots are reused, in-flight overlap):
+    every grid must equal the oracle's, bit for bit, and the stats must be per mesh."""
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    base = meshgen.make_config("cfg2")
+    meshes = [base, meshgen.carve_every_third(base), meshgen.carve_sphere(base, 0.3)]
+    for seed in (11, 12, 13):
+        meshes.append(meshgen.make_config("cfg2", seed))
+    meshes.append(Mesh("empty", base.verts, base.tets[:0], base.grid))
+    pipe = pkg.Pipe(base.grid, depth=3, max_V=max(m.V for m in meshes), max_T=max(m.T for m in meshes))
+    nx, ny, nz = base.grid
+    outs = [torch.full((1, nz, ny, nx // 32), -1, dtype=torch.int32).pin_memory() for _ in meshes]
+    tickets = [pipe.submit(_pinned(m.verts), _pinned(m.tets), o) for m, o in zip(meshes[:3], outs[:3])]
+    stats = {}
+    for k in range(3, len(meshes)):          # keep three in flight
+        stats[tickets[k - 3]] = pipe.wait(tickets[k - 3])
+        tickets.append(pipe.submit(_pinned(meshes[k].verts), _pinned(meshes[k].tets), outs[k]))
+    for t in tickets[-3:]:
+        stats[t] = pipe.wait(t)
+    assert tickets == list(range(len(meshes)))
+    for k, (m, o) in enumerate(zip(meshes, outs)):
+        assert_same(o.numpy().view(np.uint32), cpu_voxelize(m), f"pipe mesh {k} ({m.name})")
+    assert stats[len(meshes) - 1]["pairs"] == 0 and stats[0]["pairs"] > 0
+    with pytest.raises(pkg.VoxError) as ei:   # a ticket can be waited on once
+        pipe.wait(0)
+    assert ei.value.code == -5
+    pipe.close()
+
+
+def test_pipe_batched_meshes_and_limits():
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    m = meshgen.make_config("cfg3_small")
+    pipe = pkg.Pipe(m.grid, batch=m.batch, depth=2, max_V=m.V, max_T=m.T)
+    nx, ny, nz = m.grid
+    exp = cpu_voxelize(m)
+    outs = [torch.empty((m.batch, nz, ny, nx // 32), dtype=torch.int32).pin_memory() for _ in range(4)]
+    hv, ht, ho = _pinned(m.verts), _pinned(m.tets), _pinned(m.tet_offsets)
+    ts = [pipe.submit(hv, ht, o, ho) for o in outs]   # 4 submits into 2 slots: submit blocks on the oldest
+    for t in ts[2:]:
+        pipe.wait(t)
+    for o in outs:
+        assert_same(o.numpy().view(np.uint32), exp, "pipe batched")
+    big = torch.zeros((m.T + 1, 4), dtype=torch.int32).pin_memory()
+    with pytest.raises(pkg.VoxError) as ei:
+        pipe.submit(hv, big, outs[0], ho)
+    assert ei.value.code == -2
+    pipe.close()
