@@ -102,6 +102,29 @@ int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes,
  * non-empty bricks}. */
 int vox_status(vox_ctx* ctx, void* cuda_stream, const void* d_workspace, int64_t stats_out[4]);
 
+/* Sparse (two-level) output.  "voxels are often calculated and stored in
+ * octree data formats"; the binning tiles give a two-level store for free:
+ * a table with one word per tile plus the row words of the MIXED tiles only.
+ *
+ *   tile t = ((m*nbz + bz)*nby + by)*nbx + bx  covers voxels x in [32bx, 32bx+32),
+ *            y in [TY*by, TY*by+TY), z in [TZ*bz, TZ*bz+TZ) of mesh m  (vox_tile_shape gives
+ *            {TY, TZ, nbx, nby, nbz}; nbx = nx/32, nby = ceil(ny/TY), nbz = ceil(nz/TZ));
+ *   d_table[t] = 0            every voxel of the tile (inside the grid) is empty,
+ *              = 0xFFFFFFFF   every voxel of the tile (inside the grid) is solid,
+ *              = 1 + s        mixed: its row words are d_payload[s][z][y], z < TZ, y < TY
+ *                             (same bit order as the dense grid; rows outside the grid are 0),
+ *              = 0xFFFFFFFE   mixed but dropped: payload capacity exceeded (VOX_EWORKSPACE
+ *                             from vox_sparse_status / vox_pipe_wait).
+ * The slots s of the mixed tiles are a permutation of 0..mixed-1 in no particular order; the
+ * decoded grid is unique and equals vox_run's.  d_table has NB = batch*nbz*nby*nbx words,
+ * d_payload payload_capacity_tiles * TY*TZ words; d_payload may be the device view of pinned
+ * host memory.  vox_sparse_status SYNCHRONISES and returns {mixed tiles, full tiles} of the
+ * last vox_run_sparse on this workspace. */
+int vox_tile_shape(const vox_ctx* ctx, int out[5]);
+int vox_run_sparse(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes, uint32_t* d_table,
+                   uint32_t* d_payload, int64_t payload_capacity_tiles);
+int vox_sparse_status(vox_ctx* ctx, void* cuda_stream, const void* d_workspace, int64_t out[2]);
+
 /* Debug: device pass + sync; VOX_EDATA if a vertex lies outside [0,extent] or a
  * tet index outside [0,V) or the offsets are not monotone.  d_workspace needs
  * only the fixed part. */
@@ -141,9 +164,16 @@ int vox_run_host(vox_ctx* ctx, void* cuda_stream, const int32_t* h_verts, int64_
  *                     it waits for the oldest).  *ticket_out = 0,1,2,... in submit order.
  *   vox_pipe_wait     block until that mesh's grid is in h_bits_out; VOX_EWORKSPACE if
  *                     pairs were dropped (arena workspace too small for this mesh);
- *                     stats_out as vox_status (may be NULL).  Tickets may be waited once,
+ *                     stats_out (6 values, see below; may be NULL).  Tickets may be waited once,
  *                     in any order, but no later than `depth` submits after their own.
- *   vox_pipe_set_variant / vox_pipe_set_tile   as the vox_ctx calls, for every slot.
+ *   vox_pipe_submit_sparse  as vox_pipe_submit with the sparse output of vox_run_sparse:
+ *                     h_table uint32[NB] is copied out after the run; the mixed tiles are stored
+ *                     by the kernel itself straight into h_payload (pinned, device-mapped host
+ *                     memory, payload_capacity_tiles * TY*TZ words), so there is no separate
+ *                     grid copy at all.
+ *   vox_pipe_set_variant / vox_pipe_set_tile / vox_pipe_tile_shape  as the vox_ctx calls.
+ * stats_out of vox_pipe_wait: {pairs, culled tets, large-path pairs, non-empty tiles,
+ * mixed tiles, full tiles} (the last two only after a sparse submit).
  */
 typedef struct vox_pipe vox_pipe;
 int vox_pipe_create(vox_pipe** out, int nx, int ny, int nz, int ex, int ey, int ez, int batch, int depth,
@@ -155,7 +185,11 @@ size_t vox_pipe_arena_bytes(const vox_pipe* pipe);
 int vox_pipe_bind(vox_pipe* pipe, void* d_arena, size_t arena_bytes);
 int vox_pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,
                     const int64_t* h_tet_offsets, uint32_t* h_bits_out, int64_t* ticket_out);
-int vox_pipe_wait(vox_pipe* pipe, int64_t ticket, int64_t stats_out[4]);
+int vox_pipe_submit_sparse(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,
+                           const int64_t* h_tet_offsets, uint32_t* h_table, uint32_t* h_payload,
+                           int64_t payload_capacity_tiles, int64_t* ticket_out);
+int vox_pipe_wait(vox_pipe* pipe, int64_t ticket, int64_t stats_out[6]);
+int vox_pipe_tile_shape(const vox_pipe* pipe, int out[5]);
 const char* vox_pipe_last_error(const vox_pipe* pipe);
 
 /* Benchmark instrumentation (off by default).  vox_timing_enable(ctx, slots > 0)

@@ -16,6 +16,7 @@ EXPORTS = [
     "vox_probe_int32", "vox_strerror", "vox_last_error",
     "vox_pipe_create", "vox_pipe_destroy", "vox_pipe_set_variant", "vox_pipe_set_tile", "vox_pipe_arena_bytes",
     "vox_pipe_bind", "vox_pipe_submit", "vox_pipe_wait", "vox_pipe_last_error",
+    "vox_tile_shape", "vox_run_sparse", "vox_sparse_status", "vox_pipe_submit_sparse", "vox_pipe_tile_shape",
 ]
 
 
@@ -70,6 +71,11 @@ def load_library():
         "vox_pipe_submit": (i32, [vp, vp, i64, vp, i64, vp, vp, ctypes.POINTER(i64)]),
         "vox_pipe_wait": (i32, [vp, i64, ctypes.POINTER(i64)]),
         "vox_pipe_last_error": (ctypes.c_char_p, [vp]),
+        "vox_tile_shape": (i32, [vp, ctypes.POINTER(i32)]),
+        "vox_run_sparse": (i32, [vp, vp, vp, sz, vp, vp, i64]),
+        "vox_sparse_status": (i32, [vp, vp, vp, ctypes.POINTER(i64)]),
+        "vox_pipe_submit_sparse": (i32, [vp, vp, i64, vp, i64, vp, vp, vp, i64, ctypes.POINTER(i64)]),
+        "vox_pipe_tile_shape": (i32, [vp, ctypes.POINTER(i32)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -206,6 +212,44 @@ class Voxelizer:
         )
         return out
 
+    @property
+    def tile_shape(self):
+        """dict(ty, tz, nbx, nby, nbz): the binning tile (32 x ty x tz voxels) and tiles per axis."""
+        o = (ctypes.c_int * 5)()
+        self._ck(self._lib.vox_tile_shape(self._ctx, o), "vox_tile_shape")
+        return dict(ty=o[0], tz=o[1], nbx=o[2], nby=o[3], nbz=o[4])
+
+    def run_sparse(self, capacity_tiles, table=None, payload=None, stream=None):
+        """vox_run_sparse: returns (table int32[NB], payload int32[capacity][tz][ty]) CUDA tensors
+        (layout: include/vox.h).  sparse_status() gives the number of mixed tiles."""
+        torch = _torch_cuda()
+        if self._ws is None:
+            self.alloc_workspace()
+        ts = self.tile_shape
+        nb = self.batch * ts["nbx"] * ts["nby"] * ts["nbz"]
+        if table is None:
+            table = torch.empty(nb, dtype=torch.int32, device="cuda")
+        if payload is None:
+            payload = torch.empty((max(int(capacity_tiles), 1), ts["tz"], ts["ty"]), dtype=torch.int32, device="cuda")
+        assert table.is_cuda and table.numel() == nb and table.is_contiguous() and payload.is_contiguous()
+        assert payload.numel() >= int(capacity_tiles) * ts["tz"] * ts["ty"]
+        self._ck(
+            self._lib.vox_run_sparse(self._ctx, _stream_ptr(torch, stream), ctypes.c_void_p(self._ws.data_ptr()),
+                                     self._ws.numel(), ctypes.c_void_p(table.data_ptr()),
+                                     ctypes.c_void_p(payload.data_ptr()), int(capacity_tiles)),
+            "vox_run_sparse",
+        )
+        return table, payload
+
+    def sparse_status(self, stream=None):
+        """Synchronises.  dict(mixed_tiles, full_tiles); raises VoxError(-3) if payload tiles were dropped."""
+        torch = _torch_cuda()
+        o = (ctypes.c_int64 * 2)()
+        rc = self._lib.vox_sparse_status(self._ctx, _stream_ptr(torch, stream), ctypes.c_void_p(self._ws.data_ptr()), o)
+        self._last_sparse = dict(mixed_tiles=int(o[0]), full_tiles=int(o[1]))
+        self._ck(rc, "vox_sparse_status")
+        return self._last_sparse
+
     def status(self, stream=None):
         """Synchronises.  Returns dict(pairs, culled, large_pairs, nonempty_tiles); raises on overflow."""
         torch = _torch_cuda()
@@ -301,12 +345,42 @@ class Pipe:
         self._keep[ticket.value] = (h_verts, h_tets, h_out, h_tet_offsets)
         return int(ticket.value)
 
+    @property
+    def tile_shape(self):
+        o = (ctypes.c_int * 5)()
+        self._ck(self._lib.vox_pipe_tile_shape(self._p, o), "vox_pipe_tile_shape")
+        return dict(ty=o[0], tz=o[1], nbx=o[2], nby=o[3], nbz=o[4])
+
+    def submit_sparse(self, h_verts, h_tets, h_table, h_payload, capacity_tiles, h_tet_offsets=None):
+        """Sparse output (include/vox.h): h_table int32[NB] and h_payload int32[capacity][tz][ty] are pinned
+        CPU tensors; the kernel stores the mixed tiles straight into h_payload."""
+        for t in (h_verts, h_tets, h_table, h_payload) + ((h_tet_offsets,) if h_tet_offsets is not None else ()):
+            assert not t.is_cuda and t.is_contiguous() and (t.numel() == 0 or t.is_pinned()), \
+                "pipe buffers must be pinned CPU tensors"
+        ts = self.tile_shape
+        assert h_table.numel() == self.batch * ts["nbx"] * ts["nby"] * ts["nbz"]
+        assert h_payload.numel() >= int(capacity_tiles) * ts["ty"] * ts["tz"]
+        ticket = ctypes.c_int64(-1)
+        off_ptr = ctypes.c_void_p(h_tet_offsets.data_ptr()) if h_tet_offsets is not None else None
+        self._ck(
+            self._lib.vox_pipe_submit_sparse(self._p, ctypes.c_void_p(h_verts.data_ptr()), h_verts.numel() // 3,
+                                             ctypes.c_void_p(h_tets.data_ptr()), h_tets.numel() // 4, off_ptr,
+                                             ctypes.c_void_p(h_table.data_ptr()),
+                                             ctypes.c_void_p(h_payload.data_ptr()), int(capacity_tiles),
+                                             ctypes.byref(ticket)),
+            "vox_pipe_submit_sparse",
+        )
+        self._keep[ticket.value] = (h_verts, h_tets, h_table, h_payload, h_tet_offsets)
+        return int(ticket.value)
+
     def wait(self, ticket):
-        st = (ctypes.c_int64 * 4)()
+        st = (ctypes.c_int64 * 6)()
         rc = self._lib.vox_pipe_wait(self._p, int(ticket), st)
         self._keep.pop(int(ticket), None)
+        self.last_stats = dict(pairs=int(st[0]), culled=int(st[1]), large_pairs=int(st[2]), nonempty_tiles=int(st[3]),
+                               mixed_tiles=int(st[4]), full_tiles=int(st[5]))
         self._ck(rc, "vox_pipe_wait")
-        return dict(pairs=int(st[0]), culled=int(st[1]), large_pairs=int(st[2]), nonempty_tiles=int(st[3]))
+        return self.last_stats
 
     def close(self):
         if self._p:

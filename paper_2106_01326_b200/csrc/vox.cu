@@ -45,8 +45,15 @@ struct Params {
     int ex, ey, ez;
 };
 
+struct SparseOut {
+    u32* table;    // [NB]; NULL = dense output
+    u32* payload;  // [cap][TZ][TY]
+    u32 cap;       // payload capacity in tiles
+};
+
 struct vox_ctx {
     Params p;
+    SparseOut sparse;    // set for the duration of vox_run_sparse only
     bool have_tets;
     i64 pairs_planned;  // -1 = unknown
     int variant;
@@ -59,7 +66,12 @@ enum { TM_EV = 5 };  // before memset/K1, after K1, after K2, after K3, after K4
 
 enum { HDR_WORDS = 64 };
 // header words
-enum { H_TOTAL = 0, H_OVERFLOW = 1, H_CULLED = 2, H_LARGE = 3, H_NONEMPTY = 4, H_BAD = 5, H_TOTAL_HI = 6 };
+enum { H_TOTAL = 0, H_OVERFLOW = 1, H_CULLED = 2, H_LARGE = 3, H_NONEMPTY = 4, H_BAD = 5, H_TOTAL_HI = 6,
+       H_MIXED = 7, H_FULL = 8, H_PAYLOAD_OVERFLOW = 9 };
+// sparse tile table codes (include/vox.h)
+#define TILE_EMPTY 0u
+#define TILE_FULL 0xFFFFFFFFu
+#define TILE_DROPPED 0xFFFFFFFEu
 
 static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -717,10 +729,13 @@ __device__ __forceinline__ void raster_span(const int* rec, int lane, int img_st
     }
 }
 
-template <int NT, int MINB, bool UNCOND>
+// SPARSE: instead of the dense grid the CTA writes one table word for its tile (TILE_EMPTY, TILE_FULL or
+// 1 + payload slot) and, for a mixed tile only, its TY*TZ row words contiguously into payload[slot]
+// (which may be host-mapped pinned memory: the copy-out is then fused into the kernel's stores).
+template <int NT, int MINB, bool UNCOND, bool SPARSE>
 __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restrict__ offsets,
                                                     const u32* __restrict__ list, u32* __restrict__ bits,
-                                                    u32* __restrict__ hdr) {
+                                                    u32* __restrict__ hdr, SparseOut so) {
     __shared__ u32 img[32 * (32 + IMG_SKEW)];
     __shared__ __align__(16) int rec[NT][SREC_W];
     __shared__ u32 s_large;
@@ -740,6 +755,10 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
     for (int i = tid; i < img_words; i += NT) img[i] = 0;
     if (tid == 0) s_large = 0;
     const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
+    if (SPARSE && beg >= end) {  // no tets: empty tile, nothing else to do
+        if (tid == 0) so.table[b] = TILE_EMPTY;
+        return;
+    }
     u32 seen_large = 0;
     for (u32 base = beg; base < end; base += NT) {
         __syncthreads();
@@ -771,13 +790,51 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
     }
     __syncthreads();
     const int rows = 1 << (p.ty_log + p.tz_log);
+    if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
+    if (!SPARSE) {
+        for (int i = tid; i < rows; i += NT) {
+            const int z = i >> p.ty_log, y = i & (TY - 1);
+            const int gy = Y0 + y, gz = Z0 + z;
+            if (gy < p.ny && gz < p.nz)
+                bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[z * img_stride + y];
+        }
+        return;
+    }
+    // classify over the rows that lie inside the grid (ragged last tiles)
+    __shared__ u32 s_slot;
+    u32 all = 0xFFFFFFFFu, any = 0u;
     for (int i = tid; i < rows; i += NT) {
         const int z = i >> p.ty_log, y = i & (TY - 1);
-        const int gy = Y0 + y, gz = Z0 + z;
-        if (gy < p.ny && gz < p.nz)
-            bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[z * img_stride + y];
+        if (Y0 + y < p.ny && Z0 + z < p.nz) {
+            const u32 w = img[z * img_stride + y];
+            all &= w;
+            any |= w;
+        }
     }
-    if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
+    const int is_full = __syncthreads_and(all == 0xFFFFFFFFu);
+    const int is_any = __syncthreads_or(any != 0u);
+    if (!is_any || is_full) {
+        if (tid == 0) {
+            so.table[b] = is_full ? TILE_FULL : TILE_EMPTY;
+            if (is_full) atomicAdd(hdr + H_FULL, 1u);
+        }
+        return;
+    }
+    if (tid == 0) {
+        const u32 slot = atomicAdd(hdr + H_MIXED, 1u);
+        s_slot = slot;
+        so.table[b] = slot < so.cap ? slot + 1u : TILE_DROPPED;
+        if (slot >= so.cap) hdr[H_PAYLOAD_OVERFLOW] = 1;
+    }
+    __syncthreads();
+    const u32 slot = s_slot;
+    if (slot >= so.cap) return;
+    u32* dst = so.payload + (size_t)slot * rows;
+    for (int i = tid; i < rows; i += NT) {
+        const int z = i >> p.ty_log, y = i & (TY - 1);
+        const bool in = (Y0 + y < p.ny) && (Z0 + z < p.nz);
+        dst[i] = in ? img[z * img_stride + y] : 0u;
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1034,8 +1091,45 @@ extern "C" int vox_plan(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size
     return VOX_OK;
 }
 
+static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes, uint32_t* d_bits_out);
+
 extern "C" int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes, uint32_t* d_bits_out) {
     if (!ctx || !d_workspace || !d_bits_out) return VOX_EINVAL;
+    ctx->sparse = SparseOut{NULL, NULL, 0};
+    return run_impl(ctx, cuda_stream, d_workspace, ws_bytes, d_bits_out);
+}
+
+extern "C" int vox_run_sparse(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes,
+                              uint32_t* d_table, uint32_t* d_payload, int64_t payload_capacity_tiles) {
+    if (!ctx || !d_workspace || !d_table || payload_capacity_tiles < 0) return VOX_EINVAL;
+    if (payload_capacity_tiles > 0 && !d_payload) return VOX_EINVAL;
+    ctx->sparse.table = d_table;
+    ctx->sparse.payload = d_payload;
+    ctx->sparse.cap = (u32)(payload_capacity_tiles > 0xFFFFFFF0ll ? 0xFFFFFFF0ll : payload_capacity_tiles);
+    int rc = run_impl(ctx, cuda_stream, d_workspace, ws_bytes, NULL);
+    ctx->sparse = SparseOut{NULL, NULL, 0};
+    return rc;
+}
+
+extern "C" int vox_tile_shape(const vox_ctx* ctx, int out[5]) {
+    if (!ctx || !out) return VOX_EINVAL;
+    const Params& p = ctx->p;
+    out[0] = 1 << p.ty_log; out[1] = 1 << p.tz_log; out[2] = p.nbx; out[3] = p.nby; out[4] = p.nbz;
+    return VOX_OK;
+}
+
+extern "C" int vox_sparse_status(vox_ctx* ctx, void* cuda_stream, const void* d_workspace, int64_t out[2]) {
+    if (!ctx || !d_workspace) return VOX_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    WsLayout L = ws_layout(ctx->p);
+    u32 h[HDR_WORDS];
+    CK(cudaMemcpyAsync(h, (const char*)d_workspace + L.hdr, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (out) { out[0] = h[H_MIXED]; out[1] = h[H_FULL]; }
+    return (h[H_OVERFLOW] || h[H_PAYLOAD_OVERFLOW]) ? VOX_EWORKSPACE : VOX_OK;
+}
+
+static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes, uint32_t* d_bits_out) {
     if (!ctx->have_tets) return VOX_ESTATE;
     Params& p = ctx->p;
     WsLayout L = ws_layout(p);
@@ -1057,13 +1151,16 @@ extern "C" int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_
         k3_scatter<<<blocks, 256, 0, st>>>(p, range, cursor, list, hdr);
     }
     if (ev) CK(cudaEventRecord(ev[3], st));
-    switch (ctx->variant) {  // A/B variants kept for the parity tests and the sweep in DESIGN.md
+    const SparseOut so = ctx->sparse;
+    if (so.table) {
+        k4_span<128, 8, true, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);
+    } else switch (ctx->variant) {  // A/B variants kept for the parity tests and the sweep in DESIGN.md
         case 1: k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
-        case 2: k4_span<256, 4, true><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
-        case 4: k4_span<128, 8, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
-        case 5: k4_span<128, 7, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
-        case 6: k4_span<128, 9, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
-        default: k4_span<128, 8, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr);  // 64 regs, 32 warps/SM
+        case 2: k4_span<256, 4, true, false><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
+        case 4: k4_span<128, 8, false, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
+        case 5: k4_span<128, 7, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
+        case 6: k4_span<128, 9, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
+        default: k4_span<128, 8, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);  // 64 regs, 32 warps/SM
     }
     CK(cudaGetLastError());
     if (ev) {
@@ -1278,7 +1375,7 @@ extern "C" int vox_pipe_bind(vox_pipe* pipe, void* d_arena, size_t arena_bytes) 
     return VOX_OK;
 }
 
-static int pipe_finish_slot(vox_pipe* pipe, PipeSlot& s, int64_t stats_out[4]) {
+static int pipe_finish_slot(vox_pipe* pipe, PipeSlot& s, int64_t stats_out[6]) {
     PCK(cudaEventSynchronize(s.out_done));
     s.ticket = -1;
     const u32* h = s.h_hdr;
@@ -1287,12 +1384,33 @@ static int pipe_finish_slot(vox_pipe* pipe, PipeSlot& s, int64_t stats_out[4]) {
         stats_out[1] = h[H_CULLED];
         stats_out[2] = h[H_LARGE];
         stats_out[3] = h[H_NONEMPTY];
+        stats_out[4] = h[H_MIXED];
+        stats_out[5] = h[H_FULL];
     }
-    return h[H_OVERFLOW] ? VOX_EWORKSPACE : VOX_OK;
+    return (h[H_OVERFLOW] || h[H_PAYLOAD_OVERFLOW]) ? VOX_EWORKSPACE : VOX_OK;
 }
+
+static int pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,
+                       const int64_t* h_tet_offsets, uint32_t* h_bits_out, uint32_t* h_payload, int64_t cap_tiles,
+                       int64_t* ticket_out);
 
 extern "C" int vox_pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,
                                const int64_t* h_tet_offsets, uint32_t* h_bits_out, int64_t* ticket_out) {
+    return pipe_submit(pipe, h_verts, V, h_tets, T, h_tet_offsets, h_bits_out, NULL, -1, ticket_out);
+}
+
+extern "C" int vox_pipe_submit_sparse(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets,
+                                      int64_t T, const int64_t* h_tet_offsets, uint32_t* h_table,
+                                      uint32_t* h_payload, int64_t payload_capacity_tiles, int64_t* ticket_out) {
+    if (payload_capacity_tiles < 0 || (payload_capacity_tiles > 0 && !h_payload)) return VOX_EINVAL;
+    return pipe_submit(pipe, h_verts, V, h_tets, T, h_tet_offsets, h_table, h_payload, payload_capacity_tiles,
+                       ticket_out);
+}
+
+// cap_tiles < 0: dense (h_bits_out = grid); else sparse (h_bits_out = tile table, h_payload host-mapped)
+static int pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,
+                       const int64_t* h_tet_offsets, uint32_t* h_bits_out, uint32_t* h_payload, int64_t cap_tiles,
+                       int64_t* ticket_out) {
     if (!pipe || !h_bits_out || V < 0 || T < 0) return VOX_EINVAL;
     if (!pipe->bound) return VOX_ESTATE;
     if (V > pipe->maxV || T > pipe->maxT) return VOX_ERANGE;
@@ -1316,7 +1434,17 @@ extern "C" int vox_pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V
     PCK(cudaStreamWaitEvent(pipe->s_run, s.in_done, 0));
     int rc = vox_tets(ctx, (const int32_t*)(a + A.verts), V, (const int32_t*)(a + A.tets), T, (const int64_t*)(a + A.off));
     if (rc) return rc;
-    rc = vox_run(ctx, pipe->s_run, a + A.ws, pipe->slice_bytes - A.ws, (uint32_t*)(a + A.bits));
+    size_t out_bytes = vox_grid_words(ctx) * 4;
+    if (cap_tiles < 0) {
+        rc = vox_run(ctx, pipe->s_run, a + A.ws, pipe->slice_bytes - A.ws, (uint32_t*)(a + A.bits));
+    } else {
+        // the kernel stores mixed tiles straight into the caller's pinned payload buffer (device view of it)
+        void* d_payload = NULL;
+        if (cap_tiles > 0) PCK(cudaHostGetDevicePointer(&d_payload, h_payload, 0));
+        rc = vox_run_sparse(ctx, pipe->s_run, a + A.ws, pipe->slice_bytes - A.ws, (uint32_t*)(a + A.bits),
+                            (uint32_t*)d_payload, cap_tiles);
+        out_bytes = (size_t)ctx->p.NB * 4;  // the tile table lives where the dense grid would
+    }
     if (rc) {
         if (rc == VOX_ECUDA) snprintf(pipe->err, sizeof(pipe->err), "%s", ctx->err);
         return rc;
@@ -1324,7 +1452,7 @@ extern "C" int vox_pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V
     PCK(cudaEventRecord(s.run_done, pipe->s_run));
     // copy-out stream
     PCK(cudaStreamWaitEvent(pipe->s_out, s.run_done, 0));
-    PCK(cudaMemcpyAsync(h_bits_out, a + A.bits, vox_grid_words(ctx) * 4, cudaMemcpyDeviceToHost, pipe->s_out));
+    PCK(cudaMemcpyAsync(h_bits_out, a + A.bits, out_bytes, cudaMemcpyDeviceToHost, pipe->s_out));
     PCK(cudaMemcpyAsync(s.h_hdr, a + A.ws + ws_layout(ctx->p).hdr, HDR_WORDS * 4, cudaMemcpyDeviceToHost, pipe->s_out));
     PCK(cudaEventRecord(s.out_done, pipe->s_out));
     s.ticket = pipe->next_ticket++;
@@ -1332,11 +1460,15 @@ extern "C" int vox_pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V
     return VOX_OK;
 }
 
-extern "C" int vox_pipe_wait(vox_pipe* pipe, int64_t ticket, int64_t stats_out[4]) {
+extern "C" int vox_pipe_wait(vox_pipe* pipe, int64_t ticket, int64_t stats_out[6]) {
     if (!pipe || ticket < 0) return VOX_EINVAL;
     PipeSlot& s = pipe->slot[ticket % pipe->depth];
     if (s.ticket != ticket) return VOX_ESTATE;  // never submitted, already waited on, or overwritten
     return pipe_finish_slot(pipe, s, stats_out);
+}
+
+extern "C" int vox_pipe_tile_shape(const vox_pipe* pipe, int out[5]) {
+    return pipe ? vox_tile_shape(pipe->slot[0].ctx, out) : VOX_EINVAL;
 }
 
 extern "C" const char* vox_pipe_last_error(const vox_pipe* pipe) { return pipe ? pipe->err : ""; }

@@ -321,3 +321,84 @@ def test_pipe_batched_meshes_and_limits():
         pipe.submit(hv, big, outs[0], ho)
     assert ei.value.code == -2
     pipe.close()
+
+
+# ------------------------------------------------------------------ sparse output
+def _gpu_sparse(m, tile=None, capacity=None):
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    off = torch.from_numpy(m.tet_offsets).cuda() if m.batch > 1 else None
+    vz = pkg.Voxelizer(m.grid, m.extent, m.batch, tile=tile)
+    try:
+        vz.set_tets(torch.from_numpy(m.verts).cuda(), torch.from_numpy(m.tets).cuda(), off)
+        vz.plan()
+        ts = vz.tile_shape
+        nb = m.batch * ts["nbx"] * ts["nby"] * ts["nbz"]
+        cap = nb if capacity is None else capacity
+        table, payload = vz.run_sparse(cap)
+        st = vz.sparse_status()
+        return table.cpu().numpy().view(np.uint32), payload.cpu().numpy().view(np.uint32), ts, st
+    finally:
+        vz.close()
+
+
+@pytest.mark.parametrize("name,tile", [("cfg1_sphere", None), ("cfg2", None), ("cfg2", (8, 8)), ("cfg3_small", None),
+                                       ("cfg4_small_drop3", None), ("giant128_sphere", (16, 4)), ("cfg5", None)])
+def test_sparse_output_matches_oracle(name, tile):
+    from oracle import sparse
+
+    m = CASES[name]() if name in CASES else meshgen.make_config(name)
+    exp = cpu_voxelize(m)
+    table, payload, ts, st = _gpu_sparse(m, tile)
+    mixed = sparse.check_table(table, payload, exp, ts["ty"], ts["tz"])   # classes, slots, payload content
+    assert st["mixed_tiles"] == mixed
+    assert st["full_tiles"] == int(np.sum(table == np.uint32(0xFFFFFFFF)))
+    assert_same(sparse.decode(table, payload, m.grid, m.batch, ts["ty"], ts["tz"]), exp, name + " sparse decode")
+
+
+def test_sparse_ragged_grid_and_capacity_overflow():
+    import paper_2106_01326_b200 as pkg
+    from oracle import sparse
+
+    rng = np.random.default_rng(9)
+    grid, extent = (64, 20, 12), (64 * 6, 20 * 12, 12 * 18)
+    cs = [np.rint(np.linspace(0, extent[k], 4 + k)).astype(np.int64) for k in range(3)]
+    v, t = kuhn_mesh(cs[0], cs[1], cs[2], 0.2, rng)
+    t = t[rng.random(len(t)) < 0.8]
+    m = Mesh("ragged_sparse", v, t, grid, extent)
+    exp = cpu_voxelize(m)
+    for tile in [(8, 8), (16, 8), (32, 32)]:
+        table, payload, ts, st = _gpu_sparse(m, tile)
+        assert sparse.check_table(table, payload, exp, ts["ty"], ts["tz"]) == st["mixed_tiles"] > 0
+    with pytest.raises(pkg.VoxError) as ei:      # room for one payload tile only
+        _gpu_sparse(m, (8, 8), capacity=1)
+    assert ei.value.code == -3
+
+
+def test_pipe_sparse_payload_lands_in_pinned_host_memory():
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+    from oracle import sparse
+
+    base = meshgen.make_config("cfg2")
+    meshes = [base, meshgen.carve_every_third(base), meshgen.make_config("cfg2", 21), meshgen.carve_sphere(base, 0.3)]
+    pipe = pkg.Pipe(base.grid, depth=2, max_V=max(m.V for m in meshes), max_T=max(m.T for m in meshes))
+    ts = pipe.tile_shape
+    nb = ts["nbx"] * ts["nby"] * ts["nbz"]
+    tables = [torch.zeros(nb, dtype=torch.int32).pin_memory() for _ in meshes]
+    pays = [torch.zeros((nb, ts["tz"], ts["ty"]), dtype=torch.int32).pin_memory() for _ in meshes]
+    tickets, stats = [], []
+    for k, m in enumerate(meshes):
+        if k >= 2:
+            stats.append(pipe.wait(tickets[k - 2]))
+        tickets.append(pipe.submit_sparse(_pinned(m.verts), _pinned(m.tets), tables[k], pays[k], nb))
+    stats += [pipe.wait(t) for t in tickets[-2:]]
+    for k, m in enumerate(meshes):
+        exp = cpu_voxelize(m)
+        tb, pl = tables[k].numpy().view(np.uint32), pays[k].numpy().view(np.uint32)
+        assert sparse.check_table(tb, pl, exp, ts["ty"], ts["tz"]) == stats[k]["mixed_tiles"]
+        assert_same(sparse.decode(tb, pl, m.grid, 1, ts["ty"], ts["tz"]), exp, f"pipe sparse {k}")
+    pipe.close()
