@@ -360,7 +360,39 @@ def run_b200(args):
             e2e_ms = (time.perf_counter() - t0) * 1e3  # host wall clock around submit..wait of all steps
             e2e_ms = reduce_over_ranks(dist, e2e_ms, 0, 0, "cuda")[0]
             same = bool(rank != 0 or all(torch.equal(h, out.cpu()) for h in houts[:min(depth, args.e2e_steps)]))
+            # sparse output through the same pipeline (vox_pipe_submit_sparse): same steps, the grid
+            # leaves the GPU as a tile table + the mixed tiles K4 stores straight into pinned memory
+            ts = pipe.tile_shape
+            nb = m.batch * ts["nbx"] * ts["nby"] * ts["nbz"]
+            cap_tiles = int(st["nonempty_tiles"])  # a tile without tets cannot be mixed
+            htabs = [torch.zeros(nb, dtype=torch.int32).pin_memory() for _ in range(depth)]
+            hpays = [torch.zeros((cap_tiles, ts["tz"], ts["ty"]), dtype=torch.int32).pin_memory() for _ in range(depth)]
+
+            def pipe_steps_sparse(k):
+                tickets, last = [], None
+                for i in range(k):
+                    if i >= depth:
+                        pipe.wait(tickets[i - depth])
+                    tickets.append(pipe.submit_sparse(hv, ht, htabs[i % depth], hpays[i % depth], cap_tiles, ho))
+                for t in tickets[max(0, k - depth):]:
+                    last = pipe.wait(t)
+                return last
+
+            pipe_steps_sparse(max(3, depth))
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            sp_stats = pipe_steps_sparse(args.e2e_steps)
+            torch.cuda.synchronize()
+            sp_ms = (time.perf_counter() - t0) * 1e3
+            sp_ms = reduce_over_ranks(dist, sp_ms, 0, 0, "cuda")[0]
+            e2e_sparse = {"value": ssum * args.e2e_steps / (sp_ms * 1e-3) / 1e9, "unit": UNIT,
+                          "ms_per_step": sp_ms / args.e2e_steps, "h2d_bytes_per_step": None,
+                          "d2h_bytes_per_step": nb * 4 + 256 + sp_stats["mixed_tiles"] * ts["ty"] * ts["tz"] * 4,
+                          "mixed_tiles": sp_stats["mixed_tiles"], "full_tiles": sp_stats["full_tiles"], "tiles": nb,
+                          "api": f"vox_pipe_submit_sparse/vox_pipe_wait, depth {depth}; payload stored by K4 "
+                                 "into pinned host memory"}
             pipe.close()
+            del htabs, hpays
             # unpipelined single call
             vz2 = pkg.Voxelizer(m.grid, m.extent, m.batch, tile=args.tile, variant=args.variant)
             arena = torch.empty(vz2.host_arena_bytes(m.V, m.T), dtype=torch.uint8, device="cuda")
@@ -380,7 +412,9 @@ def run_b200(args):
                    "steps": args.e2e_steps, "api": f"vox_pipe_submit/vox_pipe_wait, depth {depth}",
                    "same_result": same,
                    "unpipelined_vox_run_host": {"ms_per_call": sync_ms,
-                                                "value": float(samples) / (sync_ms * 1e-3) / 1e9}}
+                                                "value": float(samples) / (sync_ms * 1e-3) / 1e9},
+                   "sparse_output": e2e_sparse}
+            e2e_sparse["h2d_bytes_per_step"] = h2d
 
         if rank != 0:
             vz.close()
@@ -440,7 +474,7 @@ def run_b200(args):
             "mtets_per_s": tsum * args.steps / sec / 1e6,
             "gvoxels_per_s": world * m.batch * nx * ny * nz * args.steps / sec / 1e9,
             "kernel_ms": shares, "status": st, "popcount": popcount,
-            "gpu_launches": 4 * (args.steps + ((args.e2e_steps + max(3, args.e2e_depth) + 5) if e2e else 0)),
+            "gpu_launches": 4 * (args.steps + ((2 * (args.e2e_steps + max(3, args.e2e_depth)) + 5) if e2e else 0)),
             "clocks": clk.summary(), "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
         }
         line["config"].pop("tile")
