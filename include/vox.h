@@ -57,12 +57,14 @@ enum {
 
 /* Grid dims in voxels (nx % 32 == 0), lattice extent per axis (extent % (2n) == 0
  * so that voxel centres are lattice points; extent <= 2^20), batch >= 1 meshes
- * sharing the grid shape.  Picks the binning tile (32 x TY x TZ voxels). */
+ * sharing the grid shape. */
 int vox_create(vox_ctx** out, int nx, int ny, int nz, int ex, int ey, int ez, int batch);
 void vox_destroy(vox_ctx* ctx);
 
-/* Optional: override the binning tile height/depth (powers of two in [4,32]).
- * Must precede vox_tets.  The result of vox_run does not depend on it. */
+/* Optional: fix the binning tile (32 x ty x tz voxels; ty, tz powers of two in [4,32]).
+ * Must precede vox_tets.  Without it vox_tets picks the tile from the grid and T (32^3
+ * bricks for big grids, thinner tiles when that leaves too few or too heavy tiles).  The
+ * result of vox_run does not depend on the tile; vox_tile_shape reports it. */
 int vox_set_tile(vox_ctx* ctx, int ty, int tz);
 
 /* Optional: kernel variant of the brick voxelizer, 0 = default.  Result-neutral
@@ -72,7 +74,8 @@ int vox_set_variant(vox_ctx* ctx, int variant);
 /* Borrow the mesh.  d_verts int32[V][3] with coordinates in [0, extent];
  * d_tets int32[T][4], indices global into d_verts; d_tet_offsets int64[batch+1]
  * (device; mesh m owns tets [off[m], off[m+1]); off[0] = 0, off[batch] = T), or
- * NULL when batch == 1.  T == 0 is legal (all-zero grid). */
+ * NULL when batch == 1.  T == 0 is legal (all-zero grid).  Picks the binning tile unless
+ * vox_set_tile fixed it (so workspace sizes and vox_tile_shape are valid after this call). */
 int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const int32_t* d_tets, int64_t T,
              const int64_t* d_tet_offsets);
 

@@ -52,6 +52,7 @@ struct SparseOut {
 };
 
 struct vox_ctx {
+    bool tile_user;      // tile fixed by vox_set_tile (or by a pipe): vox_tets does not re-pick it
     Params p;
     SparseOut sparse;    // set for the duration of vox_run_sparse only
     bool have_tets;
@@ -523,6 +524,54 @@ __device__ __noinline__ void raster_large(const Params& p, u32 t, u32 box, int X
     }
 }
 
+// the same, with the int64 planes already in the pair's shared-memory record (large_record)
+__device__ __noinline__ void raster_large_rec(const int* rec, u32* img, int lane, int img_stride) {
+    const i64* r64 = reinterpret_cast<const i64*>(rec);
+    Planes P;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        P.mx[k] = r64[k];
+        P.my[k] = r64[4 + k];
+        P.mz[k] = r64[8 + k];
+        P.g0[k] = r64[12 + k];
+    }
+    const u32 box = (u32)rec[32];
+    const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
+    const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
+    bool all_in = true, any_out = false;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        i64 ax0 = P.mx[k] * x0, ax1 = P.mx[k] * x1, ay0 = P.my[k] * y0, ay1 = P.my[k] * y1;
+        i64 az0 = P.mz[k] * z0, az1 = P.mz[k] * z1;
+        i64 lo = P.g0[k] + min(ax0, ax1) + min(ay0, ay1) + min(az0, az1);
+        i64 hi = P.g0[k] + max(ax0, ax1) + max(ay0, ay1) + max(az0, az1);
+        all_in = all_in && (lo >= 0);
+        any_out = any_out || (hi < 0);
+    }
+    if (any_out) return;  // one half-space misses the whole box: exact, G is affine
+    const u32 xmask = (0xFFFFFFFFu >> (31 - x1 + x0)) << x0;
+    const int ny = y1 - y0 + 1;
+    if (all_in) {  // the box lies inside the tet
+        const int nrows = ny * (z1 - z0 + 1);
+        for (int r = lane; r < nrows; r += 32) {
+            int zz = r / ny;
+            atomicOr(img + (z0 + zz) * img_stride + y0 + r - zz * ny, xmask);
+        }
+        return;
+    }
+    i64 c0 = P.g0[0] + P.mx[0] * lane, c1 = P.g0[1] + P.mx[1] * lane;
+    i64 c2 = P.g0[2] + P.mx[2] * lane, c3 = P.g0[3] + P.mx[3] * lane;
+    for (int z = z0; z <= z1; ++z) {
+        i64 r0 = c0 + P.mz[0] * z + P.my[0] * y0, r1 = c1 + P.mz[1] * z + P.my[1] * y0;
+        i64 r2 = c2 + P.mz[2] * z + P.my[2] * y0, r3 = c3 + P.mz[3] * z + P.my[3] * y0;
+        for (int y = y0; y <= y1; ++y) {
+            u32 word = __ballot_sync(0xFFFFFFFFu, (r0 | r1 | r2 | r3) >= 0) & xmask;
+            if (lane == 0 && word) atomicOr(img + z * img_stride + y, word);
+            r0 += P.my[0]; r1 += P.my[1]; r2 += P.my[2]; r3 += P.my[3];
+        }
+    }
+}
+
 template <int NT>
 __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__ offsets, const u32* __restrict__ list,
                                                u32* __restrict__ bits, u32* __restrict__ hdr) {
@@ -577,7 +626,7 @@ __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__
 // non-increasing in x and whose non-negative set {x : Q(x) >= 0} is
 //   hi-type (mx_G < 0): Q = G                     -> x <= b,  b = max{x : G(x) >= 0}
 //   lo-type (mx_G > 0): Q = -G - 1  (G <= -1)     -> x <= b  <=> G(x) < 0, so the half-space is x >= b+1
-//   mx_G == 0:          Q = 64*G + 63 - x (hi)    -> equivalent on x in [0,63] for integer G
+//   mx_G == 0:          r' = 64*G + 63, mx = 0 (hi) -> gates the row only (see span_plane)
 // b = floor of the real crossing r/|mx|.  A fixed-point reciprocal PROPOSES c0 = floor(r*inv/2^32), which is
 // B or B+1 for r >= 0 (see span_bound); the INTEGER value Q(c0) decides: b = c0 if Q(c0) >= 0 else c0-1.
 // No floating point at all.  Planes are stored scaled by 2 (by 4 when |mx| = 1) so that |mx| >= 4 and the
@@ -586,7 +635,8 @@ __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__
 enum { SREC_W = 36, KIND_SPAN = 0, IMG_SKEW = 11 };  // record stride 36 words: int4-aligned
 // record words: [0..3] mx  [4..7] my  [8..11] mz  [12..15] g0 (at row y0,z0)  [16..19] ceil(2^32/|mx|)
 //               [20] x0-1  [21] x1  [22] ny  [23] nrows  [24] shared byte address of image row (y0,z0)
-//               [25] div magic  [26] nlo | kind<<8  [27] tet id  [28] packed local box
+//               [25] div magic  [26] nlo  [27] tet id  [33] nlo | kind<<8
+// large records (kind = KIND_LARGE): see large_record
 // image: row (y,z) of the tile lives at img[z*(TY+IMG_SKEW) + y] (skew spreads a tet's rows over banks)
 
 // One plane of the span record.  (nx,ny,nz) = sigma*N (int32, exact), (rx,ry,rz) = Q - P0.
@@ -598,22 +648,43 @@ __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, i
     i64 mx = -(i64)nx * p.sx, my = -(i64)ny * p.sy, mz = -(i64)nz * p.sz;
     bool ok = true;
     if (mx > 0) { mx = -mx; my = -my; mz = -mz; g0 = -g0 - 1; }  // lo-type: Q = -G - 1
-    else if (mx == 0) {                                          // Q = 64*G + 63 - x
+    u32 inv;
+    if (mx == 0) {
+        // the plane does not depend on x: it only gates the row.  Stored as r' = 64*G + 63 with mx = 0 and
+        // inv = 2^31 - 1: span_bound gives c0 = floor(r'/2 - r'/2^32) >= 31 for r' >= 63 (G >= 0: not binding,
+        // x1 <= 31) and b = c0 - 1 <= -2 for r' <= -1 (G < 0: empty row).
         ok = (iabs64(g0) < (1ll << 40));
-        mx = -1; my *= 64; mz *= 64; g0 = g0 * 64 + 63;
+        my *= 64; mz *= 64; g0 = g0 * 64 + 63;
+        inv = 0x7FFFFFFFu;
+    } else {
+        // stored plane = S*Q with S*|mx| >= 4, so that the reciprocal ceil(2^32 / (S*|mx|)) fits int32
+        const int sh = (mx == -1) ? 2 : 1;
+        mx <<= sh; my <<= sh; mz <<= sh; g0 <<= sh;
+        inv = (0xFFFFFFFFu / (u32)(-mx)) + 1u;  // >= 2^32/a, < 2^32/a + 1; a >= 4 -> < 2^31
     }
-    // stored plane = S*Q with S*|mx| >= 4, so that the reciprocal ceil(2^32 / (S*|mx|)) fits int32
-    const int sh = (mx == -1) ? 2 : 1;
-    mx <<= sh; my <<= sh; mz <<= sh; g0 <<= sh;
     const i64 bound = iabs64(g0) + 34 * iabs64(mx) + 32 * (iabs64(my) + iabs64(mz));
     ok = ok && (bound < 0x7FFFFF00ll);
-    const u32 a = (u32)(-mx);
     rec[pos] = (int)mx;
     rec[4 + pos] = (int)my;
     rec[8 + pos] = (int)mz;
     rec[12 + pos] = (int)(g0 + my * y0 + mz * z0);
-    rec[16 + pos] = (int)((0xFFFFFFFFu / a) + 1u);  // >= 2^32/a, < 2^32/a + 1; a >= 4 -> < 2^31
+    rec[16 + pos] = (int)inv;
     return ok;
+}
+
+// record of a large pair: words [0..31] = int64 mx[4], my[4], mz[4], g0[4] (tet_planes), [32] packed local box
+__device__ __noinline__ void large_record(const Params& p, u32 t, int X0, int Y0, int Z0, int* rec) {
+    const Tet q = load_tet(p, t);  // reloaded here (rare path) so that the caller's copy stays in registers
+    Planes P;
+    tet_planes(p, q, X0, Y0, Z0, P);
+    i64* r64 = reinterpret_cast<i64*>(rec);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        r64[k] = P.mx[k];
+        r64[4 + k] = P.my[k];
+        r64[8 + k] = P.mz[k];
+        r64[12 + k] = P.g0[k];
+    }
 }
 
 // thread-per-(tet,tile) setup in 32-bit arithmetic.  Needs the tet's lattice bbox extent < 2^15 per
@@ -664,16 +735,22 @@ __device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0
         ok = span_plane(p, rec, pos2, s * ncx, s * ncy, s * ncz, arx, ary, arz, y0, z0) && ok;
         ok = span_plane(p, rec, pos3, -s * ndx, -s * ndy, -s * ndz, arx, ary, arz, y0, z0) && ok;
     }
+    if (!ok) {  // int64 planes for the large path, computed here (one thread per pair) rather than by a whole warp
+        large_record(p, t, X0, Y0, Z0, rec);
+        rec[32] = (int)pack_box(x0, x1, y0, y1, z0, z1);
+        rec[33] = KIND_LARGE << 8;
+        return;
+    }
     int4 a;
     a.x = x0 - 1; a.y = x1; a.z = ny; a.w = nrows;
     *reinterpret_cast<int4*>(rec + 20) = a;
     int4 b;
     b.x = (int)(img_saddr + 4u * (u32)(z0 * img_stride + y0));
     b.y = (int)((65536u + ny - 1) / ny);
-    b.z = nlo | ((ok ? KIND_SPAN : KIND_LARGE) << 8);
+    b.z = nlo;
     b.w = (int)t;
     *reinterpret_cast<int4*>(rec + 24) = b;
-    rec[28] = (int)pack_box(x0, x1, y0, y1, z0, z1);
+    rec[33] = nlo | (KIND_SPAN << 8);
 }
 
 // b = max{x : Q(x) >= 0} for Q(x) = r + mx*x, mx < 0, whenever r >= 0; some b <= -1 when r < 0.
@@ -765,12 +842,12 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
         const int n = min((u32)NT, end - base);
         if (tid < n) {
             setup_span_record(p, list[base + tid], X0, Y0, Z0, img_stride, img_saddr, rec[tid]);
-            if ((rec[tid][26] >> 8) != KIND_SPAN) atomicAdd(&s_large, 1u);
+            if ((rec[tid][33] >> 8) != KIND_SPAN) atomicAdd(&s_large, 1u);
         }
         __syncthreads();
         for (int i = warp; i < n; i += NW) {
             const int* r = rec[i];
-            const int info = r[26];
+            const int info = r[33];
             // nlo == 0 or 4 cannot happen for a non-degenerate tet (the four sigma*N sum to zero
             // and planes with N_x == 0 count as hi-type); KIND_LARGE (info >= 256) is drawn below
             if (info == 2) raster_span<2, UNCOND>(r, lane, img_stride);
@@ -783,8 +860,7 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
             seen_large = nl;
             for (int i = warp; i < n; i += NW) {
                 const int* r = rec[i];
-                if ((r[26] >> 8) != KIND_SPAN)
-                    raster_large(p, (u32)r[27], (u32)r[28], X0, Y0, Z0, img, lane, img_stride);
+                if ((r[33] >> 8) != KIND_SPAN) raster_large_rec(r, img, lane, img_stride);
             }
         }
     }
@@ -835,6 +911,215 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
         const bool in = (Y0 + y < p.ny) && (Z0 + z < p.nz);
         dst[i] = in ? img[z * img_stride + y] : 0u;
     }
+}
+
+// ------------------------------------------------------------------------------------------
+// K4 v3: row-flattened span voxelizer (default).  DESIGN.md "Kernels / K4 flat".
+// Same records and the same exact row-span arithmetic as k4_span, but the rows of a batch of NT
+// (tet,tile) pairs are laid end to end and dealt out in equal runs: thread i draws rows
+// [i*R, (i+1)*R) of the batch, whichever pairs they belong to, stepping to the next pair's record when
+// one ends.  Every lane is busy whatever the pairs' sizes are (a pair clipped to 9 rows used to occupy a
+// whole warp for one pass), and the four warps of the CTA finish together.
+// ------------------------------------------------------------------------------------------
+struct LaneRec {
+    int4 MX, MY, MZ, G0, IV, A;  // A = x0-1, x1, ny, nrows
+    int saddr, magic;
+    bool p1, p2;                 // plane 1 / plane 2 is lo-type (nlo >= 2 / nlo == 3)
+};
+
+__device__ __forceinline__ void lane_load(const int* rec, LaneRec& L) {
+    L.MX = *reinterpret_cast<const int4*>(rec);
+    L.MY = *reinterpret_cast<const int4*>(rec + 4);
+    L.MZ = *reinterpret_cast<const int4*>(rec + 8);
+    L.G0 = *reinterpret_cast<const int4*>(rec + 12);
+    L.IV = *reinterpret_cast<const int4*>(rec + 16);
+    L.A = *reinterpret_cast<const int4*>(rec + 20);
+    const int4 B = *reinterpret_cast<const int4*>(rec + 24);
+    L.saddr = B.x;
+    L.magic = B.y;
+    const int nlo = B.z & 255;
+    L.p1 = nlo >= 2;
+    L.p2 = nlo == 3;
+}
+
+// one row rr of the pair held in L: the four exact bounds, the span, one OR into the tile image
+__device__ __forceinline__ void lane_row(const LaneRec& L, int rr, int img_stride) {
+    const int zz = (int)(((u32)rr * (u32)L.magic) >> 16);
+    const int yy = rr - zz * L.A.z;
+    const int b0 = span_bound(L.G0.x + L.MY.x * yy + L.MZ.x * zz, L.MX.x, L.IV.x);
+    const int b1 = span_bound(L.G0.y + L.MY.y * yy + L.MZ.y * zz, L.MX.y, L.IV.y);
+    const int b2 = span_bound(L.G0.z + L.MY.z * yy + L.MZ.z * zz, L.MX.z, L.IV.z);
+    const int b3 = span_bound(L.G0.w + L.MY.w * yy + L.MZ.w * zz, L.MX.w, L.IV.w);
+    // planes are stored lo-types first: plane 0 is always lo, plane 3 always hi; |b| <= 2^29
+    const int NEG = -(1 << 30), POS = 1 << 30;
+    const int l1 = L.p1 ? b1 : NEG, u1 = L.p1 ? POS : b1;
+    const int l2 = L.p2 ? b2 : NEG, u2 = L.p2 ? POS : b2;
+    const int lower = max(max(L.A.x, b0), max(l1, l2));  // (first solid x) - 1
+    const int upper = min(min(L.A.y, b3), min(u1, u2));
+    const int n = upper - lower;
+    const u32 saddr = (u32)L.saddr + 4u * (u32)(zz * img_stride + yy);
+    // branch-free: PTX shifts clamp at 32, so n <= 0 gives word 0 and the OR is a no-op
+    asm volatile(
+        "{\n\t.reg .b32 m, s;\n\t"
+        "sub.s32 s, 32, %1;\n\t"
+        "shr.b32 m, 0xFFFFFFFF, s;\n\t"
+        "add.s32 s, %2, 1;\n\t"
+        "shl.b32 m, m, s;\n\t"
+        "red.shared.or.b32 [%0], m;\n\t}"
+        ::"r"(saddr), "r"(n), "r"(lower)
+        : "memory");
+}
+
+template <int NT, bool SPARSE>
+__device__ __forceinline__ void tile_epilogue(const Params& p, const u32* img, int img_stride, u32 b, u32 bx, u32 m,
+                                              int Y0, int Z0, u32* __restrict__ bits, u32* __restrict__ hdr,
+                                              const SparseOut& so, int tid) {
+    const int TY = 1 << p.ty_log;
+    const int rows = 1 << (p.ty_log + p.tz_log);
+    if (!SPARSE) {
+        for (int i = tid; i < rows; i += NT) {
+            const int z = i >> p.ty_log, y = i & (TY - 1);
+            const int gy = Y0 + y, gz = Z0 + z;
+            if (gy < p.ny && gz < p.nz)
+                bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[z * img_stride + y];
+        }
+        return;
+    }
+    // classify over the rows that lie inside the grid (ragged last tiles)
+    __shared__ u32 s_slot;
+    u32 all = 0xFFFFFFFFu, any = 0u;
+    for (int i = tid; i < rows; i += NT) {
+        const int z = i >> p.ty_log, y = i & (TY - 1);
+        if (Y0 + y < p.ny && Z0 + z < p.nz) {
+            const u32 w = img[z * img_stride + y];
+            all &= w;
+            any |= w;
+        }
+    }
+    const int is_full = __syncthreads_and(all == 0xFFFFFFFFu);
+    const int is_any = __syncthreads_or(any != 0u);
+    if (!is_any || is_full) {
+        if (tid == 0) {
+            so.table[b] = is_full ? TILE_FULL : TILE_EMPTY;
+            if (is_full) atomicAdd(hdr + H_FULL, 1u);
+        }
+        return;
+    }
+    if (tid == 0) {
+        const u32 slot = atomicAdd(hdr + H_MIXED, 1u);
+        s_slot = slot;
+        so.table[b] = slot < so.cap ? slot + 1u : TILE_DROPPED;
+        if (slot >= so.cap) hdr[H_PAYLOAD_OVERFLOW] = 1;
+    }
+    __syncthreads();
+    const u32 slot = s_slot;
+    if (slot >= so.cap) return;
+    u32* dst = so.payload + (size_t)slot * rows;
+    for (int i = tid; i < rows; i += NT) {
+        const int z = i >> p.ty_log, y = i & (TY - 1);
+        const bool in = (Y0 + y < p.ny) && (Z0 + z < p.nz);
+        dst[i] = in ? img[z * img_stride + y] : 0u;
+    }
+}
+
+template <int NT, int MINB, bool SPARSE>
+__global__ void __launch_bounds__(NT, MINB) k4_flat(Params p, const u32* __restrict__ offsets,
+                                                    const u32* __restrict__ list, u32* __restrict__ bits,
+                                                    u32* __restrict__ hdr, SparseOut so) {
+    __shared__ u32 img[32 * (32 + IMG_SKEW)];
+    __shared__ __align__(16) int rec[NT][SREC_W];
+    __shared__ int s_incl[NT];  // inclusive scan of the pairs' row counts inside each warp's 32 records
+    __shared__ int s_wtot[NT / 32];
+    __shared__ u32 s_large;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = NT / 32;
+    const u32 b = blockIdx.x;
+    const u32 bx = b % p.nbx;
+    u32 rest = b / p.nbx;
+    const u32 by = rest % p.nby;
+    rest /= p.nby;
+    const u32 bz = rest % p.nbz;
+    const u32 m = rest / p.nbz;
+    const int X0 = bx << 5, Y0 = by << p.ty_log, Z0 = bz << p.tz_log;
+    const int TY = 1 << p.ty_log, img_stride = TY + IMG_SKEW;
+    const int img_words = img_stride << p.tz_log;
+    const u32 img_saddr = (u32)__cvta_generic_to_shared(img);
+    const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
+    if (SPARSE && beg >= end) {  // no tets: empty tile, nothing else to do
+        if (tid == 0) so.table[b] = TILE_EMPTY;
+        return;
+    }
+    for (int i = tid; i < img_words; i += NT) img[i] = 0;
+    if (tid == 0) s_large = 0;
+    u32 seen_large = 0;
+    for (u32 base = beg; base < end; base += NT) {
+        __syncthreads();
+        const int n = min((u32)NT, end - base);
+        int nr = 0;
+        if (tid < n) {
+            setup_span_record(p, list[base + tid], X0, Y0, Z0, img_stride, img_saddr, rec[tid]);
+            const int info = rec[tid][33];
+            if ((info >> 8) != KIND_SPAN) atomicAdd(&s_large, 1u);
+            else if (info >= 1 && info <= 3) nr = rec[tid][23];
+            // (nlo == 0 or 4 cannot happen for a non-degenerate tet: the four sigma*N sum to zero and
+            //  planes with N_x == 0 count as hi-type; such a record would draw nothing)
+        }
+        int incl = nr;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        s_incl[tid] = incl;
+        if (lane == 31) s_wtot[warp] = incl;
+        __syncthreads();
+        // rows of the batch laid end to end: warp segment w covers [cum[w], cum[w+1])
+        int cum[NW + 1];
+        cum[0] = 0;
+#pragma unroll
+        for (int w = 0; w < NW; ++w) cum[w + 1] = cum[w] + s_wtot[w];
+        const int total = cum[NW];
+        const int R = (total + NT - 1) / NT;
+        const int first = tid * R;
+        int cnt = min(R, total - first);
+        if (cnt > 0) {
+            int w = 0, wb = 0;
+#pragma unroll
+            for (int k = 1; k < NW; ++k)
+                if (first >= cum[k]) { w = k; wb = cum[k]; }
+            const int local = first - wb;
+            const int* inc = s_incl + w * 32;
+            int j = 0;  // smallest j with inc[j] > local
+#pragma unroll
+            for (int step = 16; step; step >>= 1)
+                if (inc[j + step - 1] <= local) j += step;
+            int pi = w * 32 + j;
+            int rr = local - (j ? inc[j - 1] : 0);
+            LaneRec L;
+            lane_load(rec[pi], L);
+            for (;;) {
+                lane_row(L, rr, img_stride);
+                if (--cnt == 0) break;
+                if (++rr == L.A.w) {  // next pair that has rows (large-path records have none here)
+                    do { ++pi; } while (s_incl[pi] == ((pi & 31) ? s_incl[pi - 1] : 0));
+                    lane_load(rec[pi], L);
+                    rr = 0;
+                }
+            }
+        }
+        // large pairs of this batch (rare): one warp per pair, int64 ballot rasteriser
+        const u32 nl = s_large;  // cumulative; stable between the barrier above and the next one
+        if (nl != seen_large) {
+            seen_large = nl;
+            for (int i = warp; i < n; i += NW) {
+                const int* r = rec[i];
+                if ((r[33] >> 8) != KIND_SPAN) raster_large_rec(r, img, lane, img_stride);
+            }
+        }
+    }
+    __syncthreads();
+    if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
+    tile_epilogue<NT, SPARSE>(p, img, img_stride, b, bx, m, Y0, Z0, bits, hdr, so, tid);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -932,6 +1217,20 @@ static void set_tile(Params& p, int ty, int tz) {
     p.NB = (u32)((i64)p.batch * p.nbx * p.nby * p.nbz);
 }
 
+// Binning tile: 32^3 bricks for big grids; thinner tiles (down to 32 x 8 x 8) while there would be fewer than
+// four waves of CTAs (8 CTAs x 148 SMs each) or more than ~1024 tets per tile -- a tile's list is walked by ONE
+// CTA, 128 pairs at a time, so long lists on few tiles leave SMs idle.
+static void auto_tile(Params& p, i64 T) {
+    int ty = 32, tz = 32;
+    auto tiles = [&](int a, int b) { return (i64)p.batch * (p.nx / 32) * ((p.ny + a - 1) / a) * ((p.nz + b - 1) / b); };
+    while ((tiles(ty, tz) < 4 * 1184 || T / tiles(ty, tz) > 1024) && (ty > 8 || tz > 8)) {
+        if (tz >= ty && tz > 8) tz >>= 1; else ty >>= 1;
+    }
+    while (ty < 32 && (p.ny + ty - 1) / ty > 1024) ty <<= 1;
+    while (tz < 32 && (p.nz + tz - 1) / tz > 1024) tz <<= 1;
+    set_tile(p, ty, tz);
+}
+
 extern "C" int vox_create(vox_ctx** out, int nx, int ny, int nz, int ex, int ey, int ez, int batch) {
     if (!out) return VOX_EINVAL;
     *out = NULL;
@@ -950,16 +1249,8 @@ extern "C" int vox_create(vox_ctx** out, int nx, int ny, int nz, int ex, int ey,
     p.g_shift = ilog2_exact(p.g);
     p.sx = p.hx / p.g; p.sy = p.hy / p.g; p.sz = p.hz / p.g;
     p.wpr = nx / 32;
-    // tile: 32^3 bricks for big grids; thinner tiles when there would be too few CTAs for 148 SMs
-    int ty = 32, tz = 32;
-    auto tiles = [&](int a, int b) { return (i64)batch * (nx / 32) * ((ny + a - 1) / a) * ((nz + b - 1) / b); };
-    while (tiles(ty, tz) < 1184 && (ty > 8 || tz > 8)) {  // 1184 = 8 CTAs x 148 SMs
-        if (tz >= ty && tz > 8) tz >>= 1; else ty >>= 1;
-    }
-    while (ty < 32 && (ny + ty - 1) / ty > 1024) ty <<= 1;
-    while (tz < 32 && (nz + tz - 1) / tz > 1024) tz <<= 1;
-    set_tile(p, ty, tz);
-    if (tiles(ty, tz) > 0xFFFFFFF0ll) { free(c); return VOX_ERANGE; }
+    auto_tile(p, 0);
+    if ((i64)batch * (nx / 32) * p.nby * p.nbz > 0xFFFFFFF0ll) { free(c); return VOX_ERANGE; }
     c->pairs_planned = -1;
     *out = c;
     return VOX_OK;
@@ -1007,6 +1298,7 @@ extern "C" int vox_set_tile(vox_ctx* ctx, int ty, int tz) {
     if (ilog2_exact(ty) < 2 || ty > 32 || ilog2_exact(tz) < 2 || tz > 32) return VOX_EINVAL;
     if ((ctx->p.ny + ty - 1) / ty > 1024 || (ctx->p.nz + tz - 1) / tz > 1024) return VOX_ERANGE;
     set_tile(ctx->p, ty, tz);
+    ctx->tile_user = true;
     return VOX_OK;
 }
 
@@ -1028,6 +1320,7 @@ extern "C" int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const i
     ctx->p.V = V;
     ctx->p.T = T;
     ctx->p.off = (ctx->p.batch > 1) ? (const i64*)d_tet_offsets : NULL;
+    if (!ctx->tile_user) auto_tile(ctx->p, T);
     ctx->have_tets = true;
     ctx->pairs_planned = -1;
     return VOX_OK;
@@ -1153,14 +1446,17 @@ static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t w
     if (ev) CK(cudaEventRecord(ev[3], st));
     const SparseOut so = ctx->sparse;
     if (so.table) {
-        k4_span<128, 8, true, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);
+        k4_flat<128, 8, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);
     } else switch (ctx->variant) {  // A/B variants kept for the parity tests and the sweep in DESIGN.md
         case 1: k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
         case 2: k4_span<256, 4, true, false><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
         case 4: k4_span<128, 8, false, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
         case 5: k4_span<128, 7, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
         case 6: k4_span<128, 9, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
-        default: k4_span<128, 8, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);  // 64 regs, 32 warps/SM
+        case 3: k4_span<128, 8, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
+        case 7: k4_flat<128, 7, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
+        case 8: k4_flat<256, 4, false><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
+        default: k4_flat<128, 8, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);  // 64 regs, 32 warps/SM
     }
     CK(cudaGetLastError());
     if (ev) {
@@ -1225,6 +1521,7 @@ extern "C" size_t vox_host_arena_bytes(const vox_ctx* ctx, int64_t V, int64_t T)
     vox_ctx tmp = *ctx;
     tmp.p.T = T;
     tmp.pairs_planned = -1;
+    if (!tmp.tile_user) auto_tile(tmp.p, T);  // the tile vox_tets will pick for this T
     return arena_layout(ctx, V, T, vox_workspace_bytes(&tmp)).end;
 }
 
@@ -1324,6 +1621,8 @@ extern "C" int vox_pipe_create(vox_pipe** out, int nx, int ny, int nz, int ex, i
     for (int i = 0; i < depth; ++i) {
         int rc = vox_create(&pipe->slot[i].ctx, nx, ny, nz, ex, ey, ez, batch);
         if (rc) { vox_pipe_destroy(pipe); return rc; }
+        auto_tile(pipe->slot[i].ctx->p, max_T);  // one tile shape for every submit (the sparse table depends on it)
+        pipe->slot[i].ctx->tile_user = true;
         pipe->slot[i].ticket = -1;
     }
     bool ok = cudaStreamCreateWithFlags(&pipe->s_in, cudaStreamNonBlocking) == cudaSuccess &&
