@@ -340,7 +340,7 @@ def run_b200(args):
             depth = args.e2e_depth
             houts = [torch.empty((m.batch, nz, ny, nx // 32), dtype=torch.int32).pin_memory() for _ in range(depth)]
             pipe = pkg.Pipe(m.grid, m.extent, m.batch, depth=depth, max_V=m.V, max_T=m.T, tile=args.tile,
-                            variant=args.variant)
+                            variant=args.variant, max_pairs=pairs)
 
             def pipe_steps(k):
                 tickets = []
@@ -395,7 +395,8 @@ def run_b200(args):
             del htabs, hpays
             # unpipelined single call
             vz2 = pkg.Voxelizer(m.grid, m.extent, m.batch, tile=args.tile, variant=args.variant)
-            arena = torch.empty(vz2.host_arena_bytes(m.V, m.T), dtype=torch.uint8, device="cuda")
+            # vox_host_arena_bytes sizes the pair list by an estimate; add room for the planned count
+            arena = torch.empty(vz2.host_arena_bytes(m.V, m.T) + 4 * pairs, dtype=torch.uint8, device="cuda")
             for _ in range(2):
                 vz2.run_host(hv, ht, houts[0], arena, ho, stream)
             torch.cuda.synchronize()
@@ -441,9 +442,9 @@ def run_b200(args):
         hbm_peak = peaks.get("hbm_gbs", 6650.0)
         min_bytes = 16.0 * m.T + 12.0 * m.V + 4.0 * vz.grid_words
         k4_bytes = 4.0 * vz.grid_words + pairs * (4.0 + 16.0 + 48.0)  # grid + per pair: id, tet, 4 verts
-        tr = ncu_traffic(args.workload, "k4_span")
+        tr = ncu_traffic(args.workload, "k4_flat")
         roofline = {
-            "bound": "alu", "kernel": "k4_span", "achieved": achieved, "peak": peak_alu, "unit": "Tops/s (INT32)",
+            "bound": "alu", "kernel": "k4_flat", "achieved": achieved, "peak": peak_alu, "unit": "Tops/s (INT32)",
             "frac": achieved / peak_alu, "traffic": (tr or {}).get("bytes"), "traffic_source": (tr or {}).get("source"),
             "model": f"{OPS_PER_SAMPLE:g} ops/candidate sample + {OPS_PER_PAIR:g} ops/(tet,tile) pair",
             "ops_per_launch": ops, "kernel_ms": k4,

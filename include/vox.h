@@ -158,6 +158,9 @@ int vox_run_host(vox_ctx* ctx, void* cuda_stream, const int32_t* h_verts, int64_
  *                     outside any timed region).
  *   vox_pipe_arena_bytes  device bytes the caller must provide (depth x [verts, tets,
  *                     offsets, grid, estimated-pairs workspace]).
+ *   vox_pipe_reserve_pairs  optional, before vox_pipe_bind: size every slot's pair list for
+ *                     max_pairs (tet, tile) pairs instead of the estimate 4*max_T + tiles (meshes
+ *                     of large tets on small tiles exceed it; vox_plan gives the exact number).
  *   vox_pipe_bind     hand over the caller's device arena (borrowed until destroy).
  *   vox_pipe_submit   enqueue one mesh: H2D of h_verts int32[V][3], h_tets int32[T][4],
  *                     h_tet_offsets int64[batch+1] (NULL if batch == 1), the hot path,
@@ -184,6 +187,7 @@ int vox_pipe_create(vox_pipe** out, int nx, int ny, int nz, int ex, int ey, int 
 void vox_pipe_destroy(vox_pipe* pipe);
 int vox_pipe_set_variant(vox_pipe* pipe, int variant);
 int vox_pipe_set_tile(vox_pipe* pipe, int ty, int tz);
+int vox_pipe_reserve_pairs(vox_pipe* pipe, int64_t max_pairs);
 size_t vox_pipe_arena_bytes(const vox_pipe* pipe);
 int vox_pipe_bind(vox_pipe* pipe, void* d_arena, size_t arena_bytes);
 int vox_pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,

@@ -17,6 +17,7 @@ EXPORTS = [
     "vox_pipe_create", "vox_pipe_destroy", "vox_pipe_set_variant", "vox_pipe_set_tile", "vox_pipe_arena_bytes",
     "vox_pipe_bind", "vox_pipe_submit", "vox_pipe_wait", "vox_pipe_last_error",
     "vox_tile_shape", "vox_run_sparse", "vox_sparse_status", "vox_pipe_submit_sparse", "vox_pipe_tile_shape",
+    "vox_pipe_reserve_pairs",
 ]
 
 
@@ -76,6 +77,7 @@ def load_library():
         "vox_sparse_status": (i32, [vp, vp, vp, ctypes.POINTER(i64)]),
         "vox_pipe_submit_sparse": (i32, [vp, vp, i64, vp, i64, vp, vp, vp, i64, ctypes.POINTER(i64)]),
         "vox_pipe_tile_shape": (i32, [vp, ctypes.POINTER(i32)]),
+        "vox_pipe_reserve_pairs": (i32, [vp, i64]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -305,7 +307,8 @@ class Pipe:
     int64[batch+1]) and a pinned CPU output tensor int32[batch][nz][ny][nx/32]; wait(ticket)
     blocks until that output is complete and returns the run's statistics."""
 
-    def __init__(self, grid, extent=(65536, 65536, 65536), batch=1, depth=3, max_V=0, max_T=0, tile=None, variant=0):
+    def __init__(self, grid, extent=(65536, 65536, 65536), batch=1, depth=3, max_V=0, max_T=0, tile=None, variant=0,
+                 max_pairs=None):
         torch = _torch_cuda()
         self._lib = load_library()
         self._p = ctypes.c_void_p()
@@ -319,6 +322,8 @@ class Pipe:
             self._ck(self._lib.vox_pipe_set_tile(self._p, int(tile[0]), int(tile[1])), "vox_pipe_set_tile")
         if variant:
             self._ck(self._lib.vox_pipe_set_variant(self._p, int(variant)), "vox_pipe_set_variant")
+        if max_pairs is not None:
+            self._ck(self._lib.vox_pipe_reserve_pairs(self._p, int(max_pairs)), "vox_pipe_reserve_pairs")
         self.arena_bytes = int(self._lib.vox_pipe_arena_bytes(self._p))
         self._arena = torch.empty(self.arena_bytes + 256, dtype=torch.uint8, device="cuda")
         base = self._arena.data_ptr()

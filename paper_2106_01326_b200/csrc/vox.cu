@@ -1561,6 +1561,7 @@ struct PipeSlot {
 struct vox_pipe {
     int depth;
     i64 maxV, maxT;
+    i64 reserve_pairs;   // > 0: pair-list capacity per slot asked for by vox_pipe_reserve_pairs
     i64 next_ticket;
     cudaStream_t s_in, s_run, s_out;
     PipeSlot slot[PIPE_MAX_DEPTH];
@@ -1583,7 +1584,7 @@ static int pipe_fail(vox_pipe* q, cudaError_t e, const char* where) {
 static void pipe_layout(vox_pipe* q) {
     vox_ctx tmp = *q->slot[0].ctx;
     tmp.p.T = q->maxT;
-    tmp.pairs_planned = -1;
+    tmp.pairs_planned = q->reserve_pairs > 0 ? q->reserve_pairs : -1;
     q->A = arena_layout(&tmp, q->maxV, q->maxT, vox_workspace_bytes(&tmp));
     q->slice_bytes = align256(q->A.end);
 }
@@ -1654,6 +1655,14 @@ extern "C" int vox_pipe_set_tile(vox_pipe* pipe, int ty, int tz) {
         int rc = vox_set_tile(pipe->slot[i].ctx, ty, tz);
         if (rc) return rc;
     }
+    pipe_layout(pipe);
+    return VOX_OK;
+}
+
+extern "C" int vox_pipe_reserve_pairs(vox_pipe* pipe, int64_t max_pairs) {
+    if (!pipe || max_pairs < 0 || max_pairs > 0xFFFFFFF0ll) return VOX_EINVAL;
+    if (pipe->bound) return VOX_ESTATE;
+    pipe->reserve_pairs = max_pairs;
     pipe_layout(pipe);
     return VOX_OK;
 }
