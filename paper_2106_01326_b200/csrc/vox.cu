@@ -634,18 +634,20 @@ __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__
 // ------------------------------------------------------------------------------------------
 enum { SREC_W = 36, KIND_SPAN = 0, IMG_SKEW = 11 };  // record stride 36 words: int4-aligned
 // record words: [0..3] mx  [4..7] my  [8..11] mz  [12..15] g0 (at row y0,z0)  [16..19] ceil(2^32/|mx|)
-//               [20] x0-1  [21] x1  [22] ny  [23] nrows  [24] shared byte address of image row (y0,z0)
+//               [20] x0+1  [21] x1-x0  [22] ny  [23] nrows  [24] shared byte address of image row (y0,z0)
 //               [25] div magic  [26] nlo  [27] tet id  [33] nlo | kind<<8
 // large records (kind = KIND_LARGE): see large_record
 // image: row (y,z) of the tile lives at img[z*(TY+IMG_SKEW) + y] (skew spreads a tet's rows over banks)
 
 // One plane of the span record.  (nx,ny,nz) = sigma*N (int32, exact), (rx,ry,rz) = Q - P0.
 // G(j) = floor(C/g) - sum_a (sigma*N_a*s_a) j_a, C = sigma*N.(Q-P0)
+// The record is written relative to the pair's local box: row (yy,zz), x' = x - x0, so that the stored
+// values are distances from the BOX (not the tile) origin and small tets stay in int32 on coarse lattices.
 __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, int nx, int ny, int nz, int rx, int ry,
-                                           int rz, int y0, int z0) {
+                                           int rz, int x0, int y0, int z0, int wy, int wz) {
     const i64 C = (i64)nx * rx + (i64)ny * ry + (i64)nz * rz;
-    i64 g0 = C >> p.g_shift;
     i64 mx = -(i64)nx * p.sx, my = -(i64)ny * p.sy, mz = -(i64)nz * p.sz;
+    i64 g0 = (C >> p.g_shift) + mx * x0 + my * y0 + mz * z0;  // G at the box origin
     bool ok = true;
     if (mx > 0) { mx = -mx; my = -my; mz = -mz; g0 = -g0 - 1; }  // lo-type: Q = -G - 1
     u32 inv;
@@ -658,16 +660,20 @@ __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, i
         inv = 0x7FFFFFFFu;
     } else {
         // stored plane = S*Q with S*|mx| >= 4, so that the reciprocal ceil(2^32 / (S*|mx|)) fits int32
-        const int sh = (mx == -1) ? 2 : 1;
-        mx <<= sh; my <<= sh; mz <<= sh; g0 <<= sh;
+        // |mx| == 1 is tested on the 32-bit inputs: ptxas 12.9 (-O1 and up) folds the equivalent 64-bit test
+        // `mx == -1` at this point to false (found by the parity suite; -Xptxas -O0 gets it right)
+        const bool unit = (nx == 1 || nx == -1) && p.sx == 1;
+        const i64 S = unit ? 4 : 2;
+        mx *= S; my *= S; mz *= S; g0 *= S;
         inv = (0xFFFFFFFFu / (u32)(-mx)) + 1u;  // >= 2^32/a, < 2^32/a + 1; a >= 4 -> < 2^31
     }
-    const i64 bound = iabs64(g0) + 34 * iabs64(mx) + 32 * (iabs64(my) + iabs64(mz));
+    // every row value r of the box and r +- 2*mx (span_bound's product and check) must fit int32
+    const i64 bound = iabs64(g0) + 2 * iabs64(mx) + wy * iabs64(my) + wz * iabs64(mz);
     ok = ok && (bound < 0x7FFFFF00ll);
     rec[pos] = (int)mx;
     rec[4 + pos] = (int)my;
     rec[8 + pos] = (int)mz;
-    rec[12 + pos] = (int)(g0 + my * y0 + mz * z0);
+    rec[12 + pos] = (int)g0;
     rec[16 + pos] = (int)inv;
     return ok;
 }
@@ -730,10 +736,10 @@ __device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0
         const int pos1 = l1 ? (int)l0 : nlo + (int)!l0;
         const int pos2 = l2 ? (int)l0 + (int)l1 : nlo + (int)!l0 + (int)!l1;
         const int pos3 = l3 ? nlo - 1 : 3;
-        ok = span_plane(p, rec, pos0, s * nax, s * nay, s * naz, brx, bry, brz, y0, z0) && ok;
-        ok = span_plane(p, rec, pos1, -s * nbx, -s * nby, -s * nbz, arx, ary, arz, y0, z0) && ok;
-        ok = span_plane(p, rec, pos2, s * ncx, s * ncy, s * ncz, arx, ary, arz, y0, z0) && ok;
-        ok = span_plane(p, rec, pos3, -s * ndx, -s * ndy, -s * ndz, arx, ary, arz, y0, z0) && ok;
+        ok = span_plane(p, rec, pos0, s * nax, s * nay, s * naz, brx, bry, brz, x0, y0, z0, ny, z1 - z0 + 1) && ok;
+        ok = span_plane(p, rec, pos1, -s * nbx, -s * nby, -s * nbz, arx, ary, arz, x0, y0, z0, ny, z1 - z0 + 1) && ok;
+        ok = span_plane(p, rec, pos2, s * ncx, s * ncy, s * ncz, arx, ary, arz, x0, y0, z0, ny, z1 - z0 + 1) && ok;
+        ok = span_plane(p, rec, pos3, -s * ndx, -s * ndy, -s * ndz, arx, ary, arz, x0, y0, z0, ny, z1 - z0 + 1) && ok;
     }
     if (!ok) {  // int64 planes for the large path, computed here (one thread per pair) rather than by a whole warp
         large_record(p, t, X0, Y0, Z0, rec);
@@ -742,7 +748,7 @@ __device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0
         return;
     }
     int4 a;
-    a.x = x0 - 1; a.y = x1; a.z = ny; a.w = nrows;
+    a.x = x0 + 1; a.y = x1 - x0; a.z = ny; a.w = nrows;  // shift of the row word, box-relative x1
     *reinterpret_cast<int4*>(rec + 20) = a;
     int4 b;
     b.x = (int)(img_saddr + 4u * (u32)(z0 * img_stride + y0));
@@ -774,7 +780,7 @@ __device__ __forceinline__ void raster_span(const int* rec, int lane, int img_st
     const int4 MZ = *reinterpret_cast<const int4*>(rec + 8);
     const int4 G0 = *reinterpret_cast<const int4*>(rec + 12);
     const int4 IV = *reinterpret_cast<const int4*>(rec + 16);
-    const int4 A = *reinterpret_cast<const int4*>(rec + 20);  // x0-1, x1, ny, nrows
+    const int4 A = *reinterpret_cast<const int4*>(rec + 20);  // x0+1, x1-x0, ny, nrows
     const int2 B = *reinterpret_cast<const int2*>(rec + 24);  // shared byte address of row (y0,z0), div magic
     for (int r = lane; r < A.w; r += 32) {
         const int zz = (int)(((u32)r * (u32)B.y) >> 16);
@@ -784,9 +790,9 @@ __device__ __forceinline__ void raster_span(const int* rec, int lane, int img_st
         const int b2 = span_bound(G0.z + MY.z * yy + MZ.z * zz, MX.z, IV.z);
         const int b3 = span_bound(G0.w + MY.w * yy + MZ.w * zz, MX.w, IV.w);
         int lower, upper;  // lower = (first solid x) - 1
-        if (NLO == 1) { lower = max(A.x, b0); upper = min(min(A.y, b1), min(b2, b3)); }
-        else if (NLO == 2) { lower = max(A.x, max(b0, b1)); upper = min(A.y, min(b2, b3)); }
-        else { lower = max(max(A.x, b0), max(b1, b2)); upper = min(A.y, b3); }
+        if (NLO == 1) { lower = max(-1, b0); upper = min(min(A.y, b1), min(b2, b3)); }
+        else if (NLO == 2) { lower = max(-1, max(b0, b1)); upper = min(A.y, min(b2, b3)); }
+        else { lower = max(max(-1, b0), max(b1, b2)); upper = min(A.y, b3); }
         const int n = upper - lower;  // number of solid voxels in the row (<= 0: none)
         const u32 saddr = (u32)B.x + 4u * (u32)(zz * img_stride + yy);
         if (UNCOND) {
@@ -795,13 +801,13 @@ __device__ __forceinline__ void raster_span(const int* rec, int lane, int img_st
                 "{\n\t.reg .b32 m, s;\n\t"
                 "sub.s32 s, 32, %1;\n\t"
                 "shr.b32 m, 0xFFFFFFFF, s;\n\t"
-                "add.s32 s, %2, 1;\n\t"
+                "add.s32 s, %2, %3;\n\t"
                 "shl.b32 m, m, s;\n\t"
                 "red.shared.or.b32 [%0], m;\n\t}"
-                ::"r"(saddr), "r"(n), "r"(lower)
+                ::"r"(saddr), "r"(n), "r"(lower), "r"(A.x)
                 : "memory");
         } else if (n > 0) {
-            smem_or(saddr, (0xFFFFFFFFu >> (32 - n)) << (lower + 1));
+            smem_or(saddr, (0xFFFFFFFFu >> (32 - n)) << (lower + A.x));
         }
     }
 }
@@ -922,7 +928,7 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
 // whole warp for one pass), and the four warps of the CTA finish together.
 // ------------------------------------------------------------------------------------------
 struct LaneRec {
-    int4 MX, MY, MZ, G0, IV, A;  // A = x0-1, x1, ny, nrows
+    int4 MX, MY, MZ, G0, IV, A;  // A = x0+1, x1-x0, ny, nrows
     int saddr, magic;
     bool p1, p2;                 // plane 1 / plane 2 is lo-type (nlo >= 2 / nlo == 3)
 };
@@ -954,7 +960,7 @@ __device__ __forceinline__ void lane_row(const LaneRec& L, int rr, int img_strid
     const int NEG = -(1 << 30), POS = 1 << 30;
     const int l1 = L.p1 ? b1 : NEG, u1 = L.p1 ? POS : b1;
     const int l2 = L.p2 ? b2 : NEG, u2 = L.p2 ? POS : b2;
-    const int lower = max(max(L.A.x, b0), max(l1, l2));  // (first solid x) - 1
+    const int lower = max(max(-1, b0), max(l1, l2));  // (first solid x') - 1, x' = x - x0
     const int upper = min(min(L.A.y, b3), min(u1, u2));
     const int n = upper - lower;
     const u32 saddr = (u32)L.saddr + 4u * (u32)(zz * img_stride + yy);
@@ -963,10 +969,10 @@ __device__ __forceinline__ void lane_row(const LaneRec& L, int rr, int img_strid
         "{\n\t.reg .b32 m, s;\n\t"
         "sub.s32 s, 32, %1;\n\t"
         "shr.b32 m, 0xFFFFFFFF, s;\n\t"
-        "add.s32 s, %2, 1;\n\t"
+        "add.s32 s, %2, %3;\n\t"
         "shl.b32 m, m, s;\n\t"
         "red.shared.or.b32 [%0], m;\n\t}"
-        ::"r"(saddr), "r"(n), "r"(lower)
+        ::"r"(saddr), "r"(n), "r"(lower), "r"(L.A.x)
         : "memory");
 }
 

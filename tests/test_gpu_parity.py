@@ -95,11 +95,12 @@ def test_parity_is_tile_independent(name, tile):
     assert_same(gpu_voxelize(m, tile=tile), cpu_voxelize(m), f"{name} tile={tile}")
 
 
+@pytest.mark.parametrize("variant", [1, 3])
 @pytest.mark.parametrize("name", ["cfg1_sphere", "cfg2", "cfg4_small_drop3", "giant128_sphere", "giant256_nojit"])
-def test_parity_walker_variant(name):
-    # variant 1 = the x-walk voxelizer kept for A/B comparison; same bits
+def test_parity_kernel_variants(name, variant):
+    # variant 1 = the x-walk voxelizer, 3 = the warp-per-pair span voxelizer, kept for A/B comparison; same bits
     m = CASES[name]()
-    assert_same(gpu_voxelize(m, variant=1), cpu_voxelize(m), f"{name} variant=1")
+    assert_same(gpu_voxelize(m, variant=variant), cpu_voxelize(m), f"{name} variant={variant}")
 
 
 def test_estimated_workspace_path():
@@ -402,3 +403,30 @@ def test_pipe_sparse_payload_lands_in_pinned_host_memory():
         assert sparse.check_table(tb, pl, exp, ts["ty"], ts["tz"]) == stats[k]["mixed_tiles"]
         assert_same(sparse.decode(tb, pl, m.grid, 1, ts["ty"], ts["tz"]), exp, f"pipe sparse {k}")
     pipe.close()
+
+
+def test_planes_with_unit_and_zero_x_normal_component():
+    """Faces whose normal has x-component 0, +-1 or +-2 (the reciprocal's corner cases: |mx| = 1 is stored
+    scaled by 4, mx = 0 only gates the row).  Includes the tet that exposed a ptxas folding of `mx == -1`."""
+    rng = np.random.default_rng(2126)
+    verts = [[13118, 38472, 44237], [13629, 37852, 46741], [13779, 40783, 46370], [16778, 40704, 46380]]
+    tets = [[0, 1, 2, 3]]
+    for i in range(300):
+        a = rng.integers(6000, 50000, 3)
+        p, q = int(rng.integers(800, 4000)), int(rng.integers(-4000, 4000))
+        k = int(rng.integers(-3, 4))
+        c = int(rng.integers(0, 3))               # x-component of u x v = c  (u = (p,c,0), v = (q,k,1))
+        u, v = np.array([p, c, 0]), np.array([q, k, 1])
+        if i % 3 == 1:
+            u, v = v, u                           # -> x-component = -c
+        d = rng.integers(-6000, 6000, 3)
+        base = len(verts)
+        verts += [a.tolist(), (a + u).tolist(), (a + v).tolist(), (a + d).tolist()]
+        tets.append([base, base + 1, base + 2, base + 3])
+    m = Mesh("unit_nx", np.array(verts, dtype=np.int32), np.array(tets, dtype=np.int32), (64, 64, 64))
+    exp = cpu_voxelize(m)
+    assert exp.any()
+    for tile in [None, (32, 32), (8, 8)]:
+        assert_same(gpu_voxelize(m, tile=tile), exp, f"unit nx tile={tile}")
+    m2 = Mesh("unit_nx_fine", m.verts, m.tets, (256, 256, 256))
+    assert_same(gpu_voxelize(m2), cpu_voxelize(m2), "unit nx 256^3")
