@@ -663,8 +663,8 @@ __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, i
         // |mx| == 1 is tested on the 32-bit inputs: ptxas 12.9 (-O1 and up) folds the equivalent 64-bit test
         // `mx == -1` at this point to false (found by the parity suite; -Xptxas -O0 gets it right)
         const bool unit = (nx == 1 || nx == -1) && p.sx == 1;
-        const i64 S = unit ? 4 : 2;
-        mx *= S; my *= S; mz *= S; g0 *= S;
+        const int sh = unit ? 2 : 1;  // shifts on the unsigned image: well defined for negative values
+        mx = (i64)((u64)mx << sh); my = (i64)((u64)my << sh); mz = (i64)((u64)mz << sh); g0 = (i64)((u64)g0 << sh);
         inv = (0xFFFFFFFFu / (u32)(-mx)) + 1u;  // >= 2^32/a, < 2^32/a + 1; a >= 4 -> < 2^31
     }
     // every row value r of the box and r +- 2*mx (span_bound's product and check) must fit int32
