@@ -524,54 +524,6 @@ __device__ __noinline__ void raster_large(const Params& p, u32 t, u32 box, int X
     }
 }
 
-// the same, with the int64 planes already in the pair's shared-memory record (large_record)
-__device__ __noinline__ void raster_large_rec(const int* rec, u32* img, int lane, int img_stride) {
-    const i64* r64 = reinterpret_cast<const i64*>(rec);
-    Planes P;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        P.mx[k] = r64[k];
-        P.my[k] = r64[4 + k];
-        P.mz[k] = r64[8 + k];
-        P.g0[k] = r64[12 + k];
-    }
-    const u32 box = (u32)rec[32];
-    const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
-    const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
-    bool all_in = true, any_out = false;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        i64 ax0 = P.mx[k] * x0, ax1 = P.mx[k] * x1, ay0 = P.my[k] * y0, ay1 = P.my[k] * y1;
-        i64 az0 = P.mz[k] * z0, az1 = P.mz[k] * z1;
-        i64 lo = P.g0[k] + min(ax0, ax1) + min(ay0, ay1) + min(az0, az1);
-        i64 hi = P.g0[k] + max(ax0, ax1) + max(ay0, ay1) + max(az0, az1);
-        all_in = all_in && (lo >= 0);
-        any_out = any_out || (hi < 0);
-    }
-    if (any_out) return;  // one half-space misses the whole box: exact, G is affine
-    const u32 xmask = (0xFFFFFFFFu >> (31 - x1 + x0)) << x0;
-    const int ny = y1 - y0 + 1;
-    if (all_in) {  // the box lies inside the tet
-        const int nrows = ny * (z1 - z0 + 1);
-        for (int r = lane; r < nrows; r += 32) {
-            int zz = r / ny;
-            atomicOr(img + (z0 + zz) * img_stride + y0 + r - zz * ny, xmask);
-        }
-        return;
-    }
-    i64 c0 = P.g0[0] + P.mx[0] * lane, c1 = P.g0[1] + P.mx[1] * lane;
-    i64 c2 = P.g0[2] + P.mx[2] * lane, c3 = P.g0[3] + P.mx[3] * lane;
-    for (int z = z0; z <= z1; ++z) {
-        i64 r0 = c0 + P.mz[0] * z + P.my[0] * y0, r1 = c1 + P.mz[1] * z + P.my[1] * y0;
-        i64 r2 = c2 + P.mz[2] * z + P.my[2] * y0, r3 = c3 + P.mz[3] * z + P.my[3] * y0;
-        for (int y = y0; y <= y1; ++y) {
-            u32 word = __ballot_sync(0xFFFFFFFFu, (r0 | r1 | r2 | r3) >= 0) & xmask;
-            if (lane == 0 && word) atomicOr(img + z * img_stride + y, word);
-            r0 += P.my[0]; r1 += P.my[1]; r2 += P.my[2]; r3 += P.my[3];
-        }
-    }
-}
-
 template <int NT>
 __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__ offsets, const u32* __restrict__ list,
                                                u32* __restrict__ bits, u32* __restrict__ hdr) {
@@ -632,10 +584,10 @@ __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__
 // No floating point at all.  Planes are stored scaled by 2 (by 4 when |mx| = 1) so that |mx| >= 4 and the
 // reciprocal fits int32; all stored Q(x), x in [-1,32], and r +- mx fit int32 (checked in int64 at setup).
 // ------------------------------------------------------------------------------------------
-enum { SREC_W = 36, KIND_SPAN = 0, IMG_SKEW = 11 };  // record stride 36 words: int4-aligned
+enum { SREC_W = 40, KIND_SPAN = 0, IMG_SKEW = 11, R_BOX = 38, R_INFO = 39 };  // record stride 40 words: int4-aligned
 // record words: [0..3] mx  [4..7] my  [8..11] mz  [12..15] g0 (at row y0,z0)  [16..19] ceil(2^32/|mx|)
 //               [20] x0+1  [21] x1-x0  [22] ny  [23] nrows  [24] shared byte address of image row (y0,z0)
-//               [25] div magic  [26] nlo  [27] tet id  [33] nlo | kind<<8
+//               [25] div magic  [26] c1  [27] c2 (plane 1 / 2 is lo-type ? +2^30 : -2^30)  [39] nlo | kind<<8
 // large records (kind = KIND_LARGE): see large_record
 // image: row (y,z) of the tile lives at img[z*(TY+IMG_SKEW) + y] (skew spreads a tet's rows over banks)
 
@@ -678,18 +630,68 @@ __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, i
     return ok;
 }
 
-// record of a large pair: words [0..31] = int64 mx[4], my[4], mz[4], g0[4] (tet_planes), [32] packed local box
-__device__ __noinline__ void large_record(const Params& p, u32 t, int X0, int Y0, int Z0, int* rec) {
+// record of a large pair: the 16 int64 values mx[4], my[4], mz[4], g0[4] of tet_planes sit in words 0..19 and
+// 26..37 (LARGE_W); words 20..25 hold a one-row span header that draws nothing (x1' = -2), so that the row
+// walk of k4_flat can step over the pair like over any other; [38] packed local box, [39] kind.
+#define LARGE_W(i) ((i) < 10 ? 2 * (i) : 6 + 2 * (i))
+__device__ __noinline__ void large_record(const Params& p, u32 t, int X0, int Y0, int Z0, u32 img_saddr, int* rec) {
     const Tet q = load_tet(p, t);  // reloaded here (rare path) so that the caller's copy stays in registers
     Planes P;
     tet_planes(p, q, X0, Y0, Z0, P);
-    i64* r64 = reinterpret_cast<i64*>(rec);
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        r64[k] = P.mx[k];
-        r64[4 + k] = P.my[k];
-        r64[8 + k] = P.mz[k];
-        r64[12 + k] = P.g0[k];
+        *reinterpret_cast<i64*>(rec + LARGE_W(k)) = P.mx[k];
+        *reinterpret_cast<i64*>(rec + LARGE_W(4 + k)) = P.my[k];
+        *reinterpret_cast<i64*>(rec + LARGE_W(8 + k)) = P.mz[k];
+        *reinterpret_cast<i64*>(rec + LARGE_W(12 + k)) = P.g0[k];
+    }
+    rec[20] = 0; rec[21] = -2; rec[22] = 1; rec[23] = 1; rec[24] = (int)img_saddr; rec[25] = 0;
+}
+
+// the same, with the int64 planes already in the pair's shared-memory record (large_record)
+__device__ __noinline__ void raster_large_rec(const int* rec, u32* img, int lane, int img_stride) {
+    Planes P;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        P.mx[k] = *reinterpret_cast<const i64*>(rec + LARGE_W(k));
+        P.my[k] = *reinterpret_cast<const i64*>(rec + LARGE_W(4 + k));
+        P.mz[k] = *reinterpret_cast<const i64*>(rec + LARGE_W(8 + k));
+        P.g0[k] = *reinterpret_cast<const i64*>(rec + LARGE_W(12 + k));
+    }
+    const u32 box = (u32)rec[R_BOX];
+    const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
+    const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
+    bool all_in = true, any_out = false;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        i64 ax0 = P.mx[k] * x0, ax1 = P.mx[k] * x1, ay0 = P.my[k] * y0, ay1 = P.my[k] * y1;
+        i64 az0 = P.mz[k] * z0, az1 = P.mz[k] * z1;
+        i64 lo = P.g0[k] + min(ax0, ax1) + min(ay0, ay1) + min(az0, az1);
+        i64 hi = P.g0[k] + max(ax0, ax1) + max(ay0, ay1) + max(az0, az1);
+        all_in = all_in && (lo >= 0);
+        any_out = any_out || (hi < 0);
+    }
+    if (any_out) return;  // one half-space misses the whole box: exact, G is affine
+    const u32 xmask = (0xFFFFFFFFu >> (31 - x1 + x0)) << x0;
+    const int ny = y1 - y0 + 1;
+    if (all_in) {  // the box lies inside the tet
+        const int nrows = ny * (z1 - z0 + 1);
+        for (int r = lane; r < nrows; r += 32) {
+            int zz = r / ny;
+            atomicOr(img + (z0 + zz) * img_stride + y0 + r - zz * ny, xmask);
+        }
+        return;
+    }
+    i64 c0 = P.g0[0] + P.mx[0] * lane, c1 = P.g0[1] + P.mx[1] * lane;
+    i64 c2 = P.g0[2] + P.mx[2] * lane, c3 = P.g0[3] + P.mx[3] * lane;
+    for (int z = z0; z <= z1; ++z) {
+        i64 r0 = c0 + P.mz[0] * z + P.my[0] * y0, r1 = c1 + P.mz[1] * z + P.my[1] * y0;
+        i64 r2 = c2 + P.mz[2] * z + P.my[2] * y0, r3 = c3 + P.mz[3] * z + P.my[3] * y0;
+        for (int y = y0; y <= y1; ++y) {
+            u32 word = __ballot_sync(0xFFFFFFFFu, (r0 | r1 | r2 | r3) >= 0) & xmask;
+            if (lane == 0 && word) atomicOr(img + z * img_stride + y, word);
+            r0 += P.my[0]; r1 += P.my[1]; r2 += P.my[2]; r3 += P.my[3];
+        }
     }
 }
 
@@ -742,21 +744,24 @@ __device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0
         ok = span_plane(p, rec, pos3, -s * ndx, -s * ndy, -s * ndz, arx, ary, arz, x0, y0, z0, ny, z1 - z0 + 1) && ok;
     }
     if (!ok) {  // int64 planes for the large path, computed here (one thread per pair) rather than by a whole warp
-        large_record(p, t, X0, Y0, Z0, rec);
-        rec[32] = (int)pack_box(x0, x1, y0, y1, z0, z1);
-        rec[33] = KIND_LARGE << 8;
+        large_record(p, t, X0, Y0, Z0, img_saddr, rec);
+        rec[R_BOX] = (int)pack_box(x0, x1, y0, y1, z0, z1);
+        rec[R_INFO] = KIND_LARGE << 8;
         return;
     }
+    // nlo == 0 or 4 cannot happen for a non-degenerate tet (the four sigma*N sum to zero and planes with
+    // N_x == 0 count as hi-type); such a record is made to draw nothing: one row, x1' = -2
+    const bool valid = nlo >= 1 && nlo <= 3;
     int4 a;
-    a.x = x0 + 1; a.y = x1 - x0; a.z = ny; a.w = nrows;  // shift of the row word, box-relative x1
+    a.x = x0 + 1; a.y = valid ? x1 - x0 : -2; a.z = ny; a.w = valid ? nrows : 1;  // shift of the row word, box-relative x1
     *reinterpret_cast<int4*>(rec + 20) = a;
     int4 b;
     b.x = (int)(img_saddr + 4u * (u32)(z0 * img_stride + y0));
     b.y = (int)((65536u + ny - 1) / ny);
-    b.z = nlo;
-    b.w = (int)t;
+    b.z = nlo >= 2 ? (1 << 30) : -(1 << 30);   // c1
+    b.w = nlo == 3 ? (1 << 30) : -(1 << 30);   // c2
     *reinterpret_cast<int4*>(rec + 24) = b;
-    rec[33] = nlo | (KIND_SPAN << 8);
+    rec[R_INFO] = nlo | (KIND_SPAN << 8);
 }
 
 // b = max{x : Q(x) >= 0} for Q(x) = r + mx*x, mx < 0, whenever r >= 0; some b <= -1 when r < 0.
@@ -848,12 +853,12 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
         const int n = min((u32)NT, end - base);
         if (tid < n) {
             setup_span_record(p, list[base + tid], X0, Y0, Z0, img_stride, img_saddr, rec[tid]);
-            if ((rec[tid][33] >> 8) != KIND_SPAN) atomicAdd(&s_large, 1u);
+            if ((rec[tid][R_INFO] >> 8) != KIND_SPAN) atomicAdd(&s_large, 1u);
         }
         __syncthreads();
         for (int i = warp; i < n; i += NW) {
             const int* r = rec[i];
-            const int info = r[33];
+            const int info = r[R_INFO];
             // nlo == 0 or 4 cannot happen for a non-degenerate tet (the four sigma*N sum to zero
             // and planes with N_x == 0 count as hi-type); KIND_LARGE (info >= 256) is drawn below
             if (info == 2) raster_span<2, UNCOND>(r, lane, img_stride);
@@ -866,7 +871,7 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
             seen_large = nl;
             for (int i = warp; i < n; i += NW) {
                 const int* r = rec[i];
-                if ((r[33] >> 8) != KIND_SPAN) raster_large_rec(r, img, lane, img_stride);
+                if ((r[R_INFO] >> 8) != KIND_SPAN) raster_large_rec(r, img, lane, img_stride);
             }
         }
     }
@@ -930,7 +935,7 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
 struct LaneRec {
     int4 MX, MY, MZ, G0, IV, A;  // A = x0+1, x1-x0, ny, nrows
     int saddr, magic;
-    bool p1, p2;                 // plane 1 / plane 2 is lo-type (nlo >= 2 / nlo == 3)
+    int c1, c2;                  // plane 1 / plane 2 is lo-type ? +2^30 : -2^30
 };
 
 __device__ __forceinline__ void lane_load(const int* rec, LaneRec& L) {
@@ -943,9 +948,8 @@ __device__ __forceinline__ void lane_load(const int* rec, LaneRec& L) {
     const int4 B = *reinterpret_cast<const int4*>(rec + 24);
     L.saddr = B.x;
     L.magic = B.y;
-    const int nlo = B.z & 255;
-    L.p1 = nlo >= 2;
-    L.p2 = nlo == 3;
+    L.c1 = B.z;
+    L.c2 = B.w;
 }
 
 // one row rr of the pair held in L: the four exact bounds, the span, one OR into the tile image
@@ -957,9 +961,9 @@ __device__ __forceinline__ void lane_row(const LaneRec& L, int rr, int img_strid
     const int b2 = span_bound(L.G0.z + L.MY.z * yy + L.MZ.z * zz, L.MX.z, L.IV.z);
     const int b3 = span_bound(L.G0.w + L.MY.w * yy + L.MZ.w * zz, L.MX.w, L.IV.w);
     // planes are stored lo-types first: plane 0 is always lo, plane 3 always hi; |b| <= 2^29
-    const int NEG = -(1 << 30), POS = 1 << 30;
-    const int l1 = L.p1 ? b1 : NEG, u1 = L.p1 ? POS : b1;
-    const int l2 = L.p2 ? b2 : NEG, u2 = L.p2 ? POS : b2;
+    // lo-type (c = +2^30): min(b,c) = b joins the lower bounds, max(b,c) = c is no upper bound; hi-type the reverse
+    const int l1 = min(b1, L.c1), u1 = max(b1, L.c1);
+    const int l2 = min(b2, L.c2), u2 = max(b2, L.c2);
     const int lower = max(max(-1, b0), max(l1, l2));  // (first solid x') - 1, x' = x - x0
     const int upper = min(min(L.A.y, b3), min(u1, u2));
     const int n = upper - lower;
@@ -1064,11 +1068,8 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(Params p, const u32* __restr
         int nr = 0;
         if (tid < n) {
             setup_span_record(p, list[base + tid], X0, Y0, Z0, img_stride, img_saddr, rec[tid]);
-            const int info = rec[tid][33];
-            if ((info >> 8) != KIND_SPAN) atomicAdd(&s_large, 1u);
-            else if (info >= 1 && info <= 3) nr = rec[tid][23];
-            // (nlo == 0 or 4 cannot happen for a non-degenerate tet: the four sigma*N sum to zero and
-            //  planes with N_x == 0 count as hi-type; such a record would draw nothing)
+            if ((rec[tid][R_INFO] >> 8) != KIND_SPAN) atomicAdd(&s_large, 1u);
+            nr = rec[tid][23];  // >= 1 for every pair: large pairs carry a one-row header that draws nothing
         }
         int incl = nr;
 #pragma unroll
@@ -1106,9 +1107,8 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(Params p, const u32* __restr
             for (;;) {
                 lane_row(L, rr, img_stride);
                 if (--cnt == 0) break;
-                if (++rr == L.A.w) {  // next pair that has rows (large-path records have none here)
-                    do { ++pi; } while (s_incl[pi] == ((pi & 31) ? s_incl[pi - 1] : 0));
-                    lane_load(rec[pi], L);
+                if (++rr == L.A.w) {  // next pair (every pair has at least one row)
+                    lane_load(rec[++pi], L);
                     rr = 0;
                 }
             }
@@ -1119,7 +1119,7 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(Params p, const u32* __restr
             seen_large = nl;
             for (int i = warp; i < n; i += NW) {
                 const int* r = rec[i];
-                if ((r[33] >> 8) != KIND_SPAN) raster_large_rec(r, img, lane, img_stride);
+                if ((r[R_INFO] >> 8) != KIND_SPAN) raster_large_rec(r, img, lane, img_stride);
             }
         }
     }
