@@ -105,6 +105,9 @@ def ncu_traffic(workload, kernel):
             f = [x.strip() for x in ln.split(",")]
             if len(f) >= 5 and f[0] == workload and f[1] == kernel:
                 best = {"bytes": float(f[2]) + float(f[3]), "source": "profiles/" + f[4]}
+                if len(f) >= 7:  # the same capture's warp instructions and issue-slot utilisation
+                    best["ncu"] = {"warp_inst_executed": float(f[5]), "issue_active_pct": float(f[6]),
+                                   "gpu_time_ms": float(f[7]) if len(f) >= 8 else None}
         return best
     except OSError:
         return None
@@ -445,7 +448,7 @@ def run_b200(args):
         tr = ncu_traffic(args.workload, "k4_flat")
         roofline = {
             "bound": "alu", "kernel": "k4_flat", "achieved": achieved, "peak": peak_alu, "unit": "Tops/s (INT32)",
-            "frac": achieved / peak_alu, "traffic": (tr or {}).get("bytes"), "traffic_source": (tr or {}).get("source"),
+            "frac": achieved / peak_alu, "traffic": (tr or {}).get("bytes"), "traffic_source": (tr or {}).get("source"), "ncu": (tr or {}).get("ncu"),
             "model": f"{OPS_PER_SAMPLE:g} ops/candidate sample + {OPS_PER_PAIR:g} ops/(tet,tile) pair",
             "ops_per_launch": ops, "kernel_ms": k4,
             "peak_source": "derived: 148 SMs x 64 alu-pipe lanes x clocks.max.sm (DESIGN.md Roofline)",
