@@ -35,6 +35,7 @@ struct Params {
     int nx, ny, nz;
     int hx, hy, hz;      // pitch per axis
     int qx, qy, qz;      // log2(2h) per axis, or -1 when 2h is not a power of two
+    int lim_x, lim_y, lim_z;  // (2^30 - 1) / (h/g): largest |N| component whose scaled coefficient fits
     int g, g_shift;      // gcd of the pitches; log2(g) or -1
     int sx, sy, sz;      // h / g
     int ty_log, tz_log;  // tile = 32 x (1<<ty_log) x (1<<tz_log) voxels
@@ -597,35 +598,36 @@ enum { SREC_W = 40, KIND_SPAN = 0, IMG_SKEW = 11, R_BOX = 38, R_INFO = 39 };  //
 // values are distances from the BOX (not the tile) origin and small tets stay in int32 on coarse lattices.
 __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, int nx, int ny, int nz, int rx, int ry,
                                            int rz, int x0, int y0, int z0, int wy, int wz) {
+    // 64-bit only where the VALUE needs it (C and the box-origin shift); everything else is 32-bit once the
+    // coefficients are known to fit.  Anything that does not fit returns false -> exact int64 large path.
+    bool ok = (abs(nx) <= p.lim_x) && (abs(ny) <= p.lim_y) && (abs(nz) <= p.lim_z);  // |m| < 2^30
+    // (unsigned products: no signed overflow when a component is out of range and ok is already false)
+    int mx = (int)(0u - (u32)nx * (u32)p.sx), my = (int)(0u - (u32)ny * (u32)p.sy), mz = (int)(0u - (u32)nz * (u32)p.sz);
     const i64 C = (i64)nx * rx + (i64)ny * ry + (i64)nz * rz;
-    i64 mx = -(i64)nx * p.sx, my = -(i64)ny * p.sy, mz = -(i64)nz * p.sz;
-    i64 g0 = (C >> p.g_shift) + mx * x0 + my * y0 + mz * z0;  // G at the box origin
-    bool ok = true;
-    if (mx > 0) { mx = -mx; my = -my; mz = -mz; g0 = -g0 - 1; }  // lo-type: Q = -G - 1
-    u32 inv;
-    if (mx == 0) {
-        // the plane does not depend on x: it only gates the row.  Stored as r' = 64*G + 63 with mx = 0 and
-        // inv = 2^31 - 1: span_bound gives c0 = floor(r'/2 - r'/2^32) >= 31 for r' >= 63 (G >= 0: not binding,
-        // x1 <= 31) and b = c0 - 1 <= -2 for r' <= -1 (G < 0: empty row).
-        ok = (iabs64(g0) < (1ll << 40));
-        my *= 64; mz *= 64; g0 = g0 * 64 + 63;
-        inv = 0x7FFFFFFFu;
-    } else {
-        // stored plane = S*Q with S*|mx| >= 4, so that the reciprocal ceil(2^32 / (S*|mx|)) fits int32
-        // |mx| == 1 is tested on the 32-bit inputs: ptxas 12.9 (-O1 and up) folds the equivalent 64-bit test
-        // `mx == -1` at this point to false (found by the parity suite; -Xptxas -O0 gets it right)
-        const bool unit = (nx == 1 || nx == -1) && p.sx == 1;
-        const int sh = unit ? 2 : 1;  // shifts on the unsigned image: well defined for negative values
-        mx = (i64)((u64)mx << sh); my = (i64)((u64)my << sh); mz = (i64)((u64)mz << sh); g0 = (i64)((u64)g0 << sh);
-        inv = (0xFFFFFFFFu / (u32)(-mx)) + 1u;  // >= 2^32/a, < 2^32/a + 1; a >= 4 -> < 2^31
-    }
-    // every row value r of the box and r +- 2*mx (span_bound's product and check) must fit int32
-    const i64 bound = iabs64(g0) + 2 * iabs64(mx) + wy * iabs64(my) + wz * iabs64(mz);
-    ok = ok && (bound < 0x7FFFFF00ll);
-    rec[pos] = (int)mx;
-    rec[4 + pos] = (int)my;
-    rec[8 + pos] = (int)mz;
-    rec[12 + pos] = (int)g0;
+    const i64 g64 = (C >> p.g_shift) + (i64)mx * x0 + (i64)my * y0 + (i64)mz * z0;  // G at the box origin
+    ok = ok && ((u64)(g64 + (1ll << 30)) < (1ull << 31));                          // |g0| <= 2^30
+    int g0 = (int)g64;
+    if (mx > 0) { mx = (int)(0u - (u32)mx); my = (int)(0u - (u32)my); mz = (int)(0u - (u32)mz); g0 = ~g0; }  // lo-type: Q = -G - 1
+    // scale: 2 (4 when |mx| == 1) so that the reciprocal ceil(2^32 / |mx|) fits int32; a plane with mx == 0 does
+    // not depend on x and only gates the row: stored as r' = 64*G + 63 with inv = 2^31 - 1, for which span_bound
+    // gives c0 = floor(r'/2 - r'/2^32) >= 31 when r' >= 63 (G >= 0: not binding, x1' <= 31) and b = c0 - 1 <= -2
+    // when r' <= -1 (G < 0: empty row).
+    const int sh = (mx == 0) ? 6 : ((mx == -1) ? 2 : 1);
+    // every row value r of the box and r +- 2*mx (span_bound's product and check) must fit int32 after scaling
+    u64 acc = (u64)(u32)abs(g0) + 2ull * (0u - (u32)mx);
+    acc += (u64)(u32)wy * (u32)abs(my);
+    acc += (u64)(u32)wz * (u32)abs(mz);
+    ok = ok && (acc < (u64)((0x7FFFFF00u - 63u) >> sh));
+    mx = (int)((u32)mx << sh);
+    my = (int)((u32)my << sh);
+    mz = (int)((u32)mz << sh);
+    g0 = (int)((u32)g0 << sh) + ((sh == 6) ? 63 : 0);
+    const u32 a = max((u32)(-mx), 4u);  // a valid plane with mx != 0 has |mx| >= 4 after scaling
+    const u32 inv = (sh == 6) ? 0x7FFFFFFFu : (0xFFFFFFFFu / a) + 1u;  // in [2^32/a, 2^32/a + 1), < 2^31
+    rec[pos] = mx;
+    rec[4 + pos] = my;
+    rec[8 + pos] = mz;
+    rec[12 + pos] = g0;
     rec[16 + pos] = (int)inv;
     return ok;
 }
@@ -1254,6 +1256,7 @@ extern "C" int vox_create(vox_ctx** out, int nx, int ny, int nz, int ex, int ey,
     p.g = gcd_i(gcd_i(p.hx, p.hy), p.hz);
     p.g_shift = ilog2_exact(p.g);
     p.sx = p.hx / p.g; p.sy = p.hy / p.g; p.sz = p.hz / p.g;
+    p.lim_x = ((1 << 30) - 1) / p.sx; p.lim_y = ((1 << 30) - 1) / p.sy; p.lim_z = ((1 << 30) - 1) / p.sz;
     p.wpr = nx / 32;
     auto_tile(p, 0);
     if ((i64)batch * (nx / 32) * p.nby * p.nbz > 0xFFFFFFF0ll) { free(c); return VOX_ERANGE; }
