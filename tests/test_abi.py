@@ -105,3 +105,58 @@ def test_product_does_not_import_oracle():
             if f.endswith((".py", ".cu", ".h", ".cuh")):
                 s = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in s.replace("no CPU oracle", ""), f
+
+
+def _tile(lib, grid, batch, T):
+    c = ctypes.c_void_p()
+    E = 65536
+    assert lib.vox_create(ctypes.byref(c), *grid, E, E, E, batch) == 0
+    fake = ctypes.c_void_p(256)  # never dereferenced by vox_tets
+    off = fake if batch > 1 else None
+    assert lib.vox_tets(c, fake, 10, fake, T, off) == 0
+    o = (ctypes.c_int * 5)()
+    assert lib.vox_tile_shape(c, o) == 0
+    fixed = lib.vox_workspace_fixed_bytes(c)
+    lib.vox_destroy(c)
+    return tuple(o), fixed
+
+
+def test_tile_choice_depends_on_grid_and_tet_count(lib):
+    """auto_tile: 32^3 bricks for big grids, thinner tiles while there are fewer than
+    four waves of CTAs or more than ~1024 tets per tile; a tile fixed by vox_set_tile is kept."""
+    (ty, tz, nbx, nby, nbz), _ = _tile(lib, (1024, 1024, 1024), 1, 4829739)     # cfg4
+    assert (ty, tz) == (32, 32) and (nbx, nby, nbz) == (32, 32, 32)
+    (ty, tz, *_), _ = _tile(lib, (256, 256, 256), 1, 10110954)                    # 10^7 tets at 256^3: min tile
+    assert (ty, tz) == (8, 8)
+    (ty, tz, nbx, nby, nbz), _ = _tile(lib, (64, 64, 64), 256, 5271425)           # cfg3
+    assert 256 * nbx * nby * nbz >= 4 * 1184 and max(ty, tz) <= 16
+    (ty, tz, *_), _ = _tile(lib, (32, 32, 32), 1, 384)                            # cfg1: as many CTAs as possible
+    assert (ty, tz) == (8, 8)
+    small, f_small = _tile(lib, (512, 512, 512), 1, 1000)
+    big, f_big = _tile(lib, (512, 512, 512), 1, 40_000_000)
+    assert small[0] * small[1] >= big[0] * big[1] and f_big > f_small           # more tets -> thinner tiles
+    # a user-fixed tile survives vox_tets
+    c = ctypes.c_void_p()
+    assert lib.vox_create(ctypes.byref(c), 256, 256, 256, 65536, 65536, 65536, 1) == 0
+    assert lib.vox_set_tile(c, 32, 16) == 0
+    assert lib.vox_tets(c, ctypes.c_void_p(256), 10, ctypes.c_void_p(256), 10_000_000, None) == 0
+    o = (ctypes.c_int * 5)()
+    assert lib.vox_tile_shape(c, o) == 0 and (o[0], o[1]) == (32, 16)
+    lib.vox_destroy(c)
+
+
+def test_sparse_and_pipe_argument_checks(lib):
+    c = ctypes.c_void_p()
+    assert lib.vox_create(ctypes.byref(c), 64, 64, 64, 65536, 65536, 65536, 1) == 0
+    fake = ctypes.c_void_p(256)
+    assert lib.vox_run_sparse(c, None, fake, 1 << 20, None, fake, 4) == -1          # no table
+    assert lib.vox_run_sparse(c, None, fake, 1 << 20, fake, None, 4) == -1          # capacity without payload
+    assert lib.vox_run_sparse(c, None, fake, 1 << 20, fake, fake, 4) == -5          # before vox_tets
+    assert lib.vox_tile_shape(c, None) == -1
+    lib.vox_destroy(c)
+    p = ctypes.c_void_p()
+    assert lib.vox_pipe_create(ctypes.byref(p), 64, 64, 64, 65536, 65536, 65536, 1, 0, 10, 10) == -1   # depth
+    assert lib.vox_pipe_create(ctypes.byref(p), 64, 64, 64, 65536, 65536, 65536, 1, 9, 10, 10) == -1
+    assert lib.vox_pipe_create(ctypes.byref(p), 60, 64, 64, 65536, 65536, 65536, 1, 2, 10, 10) == -1   # nx % 32
+    assert not p.value
+    assert lib.vox_pipe_arena_bytes(None) == 0 and lib.vox_pipe_wait(None, 0, None) == -1
