@@ -128,6 +128,16 @@ int vox_run_sparse(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws
                    uint32_t* d_payload, int64_t payload_capacity_tiles);
 int vox_sparse_status(vox_ctx* ctx, void* cuda_stream, const void* d_workspace, int64_t out[2]);
 
+/* Occupancy from sub-samples.  The paper's comparison voxelizes "each model ... into 5
+ * million samples, with a resolution of 256^3": more than one sample per voxel.  Reading taken
+ * (DESIGN.md): k x k x k regularly spaced sub-samples per voxel = the voxel centres of a grid k times finer per
+ * axis, so the mesh is voxelized with vox_run on (k*nx, k*ny, k*nz) and this call folds that bit grid:
+ *   d_counts_out[((m*nz + z)*ny + y)*nx + x] = number of solid sub-samples of voxel (x,y,z), 0..k^3 (uint8).
+ * nx, ny, nz are the COARSE dims; k is 2 or 4; (k*nx) % 32 == 0; d_bits_fine has the vox_run layout of the fine
+ * grid.  Enqueue only (no sync, no allocation). */
+int vox_occupancy(void* cuda_stream, const uint32_t* d_bits_fine, int nx, int ny, int nz, int batch, int k,
+                  uint8_t* d_counts_out);
+
 /* Debug: device pass + sync; VOX_EDATA if a vertex lies outside [0,extent] or a
  * tet index outside [0,V) or the offsets are not monotone.  d_workspace needs
  * only the fixed part. */

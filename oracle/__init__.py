@@ -11,6 +11,9 @@ Two independent implementations of the same plain definition (DESIGN.md
     sample (``voxelize``);
   * ``bruteforce.py``   -- pure Python big integers, all voxels x all tets, no
     bounding box (tiny inputs; pins the C one).
+
+plus the plain definitions of the two derived outputs: ``sparse.py`` (two-level tile encoding) and
+``occupancy.py`` (k^3 sub-sample counts).
 """
 from .binding import (  # noqa: F401
     build,

@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     Voxelizer,
     lib_path,
     load_library,
+    occupancy,
     probe_int32,
     voxelize,
     voxelize_host,

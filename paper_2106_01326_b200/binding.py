@@ -17,7 +17,7 @@ EXPORTS = [
     "vox_pipe_create", "vox_pipe_destroy", "vox_pipe_set_variant", "vox_pipe_set_tile", "vox_pipe_arena_bytes",
     "vox_pipe_bind", "vox_pipe_submit", "vox_pipe_wait", "vox_pipe_last_error",
     "vox_tile_shape", "vox_run_sparse", "vox_sparse_status", "vox_pipe_submit_sparse", "vox_pipe_tile_shape",
-    "vox_pipe_reserve_pairs",
+    "vox_pipe_reserve_pairs", "vox_occupancy",
 ]
 
 
@@ -78,6 +78,7 @@ def load_library():
         "vox_pipe_submit_sparse": (i32, [vp, vp, i64, vp, i64, vp, vp, vp, i64, ctypes.POINTER(i64)]),
         "vox_pipe_tile_shape": (i32, [vp, ctypes.POINTER(i32)]),
         "vox_pipe_reserve_pairs": (i32, [vp, i64]),
+        "vox_occupancy": (i32, [vp, vp, i32, i32, i32, i32, i32, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -426,6 +427,23 @@ def voxelize(verts, tets, grid, extent=(65536, 65536, 65536), tet_offsets=None, 
         return res
     finally:
         vz.close()
+
+
+def occupancy(bits_fine, grid, k, batch=1, out=None, stream=None):
+    """vox_occupancy: fold a bit grid voxelized at k times `grid`'s resolution (CUDA int32 tensor
+    [batch][k*nz][k*ny][k*nx/32]) into solid sub-sample counts, CUDA uint8 [batch][nz][ny][nx]."""
+    torch = _torch_cuda()
+    lib = load_library()
+    nx, ny, nz = (int(g) for g in grid)
+    assert bits_fine.is_cuda and bits_fine.is_contiguous()
+    assert bits_fine.numel() == batch * (k * nz) * (k * ny) * (k * nx // 32)
+    if out is None:
+        out = torch.empty((batch, nz, ny, nx), dtype=torch.uint8, device="cuda")
+    rc = lib.vox_occupancy(_stream_ptr(torch, stream), ctypes.c_void_p(bits_fine.data_ptr()), nx, ny, nz, int(batch),
+                           int(k), ctypes.c_void_p(out.data_ptr()))
+    if rc:
+        raise VoxError(rc, "vox_occupancy")
+    return out
 
 
 def voxelize_host(verts, tets, grid, extent=(65536, 65536, 65536), tet_offsets=None):

@@ -1557,6 +1557,59 @@ extern "C" int vox_run_host(vox_ctx* ctx, void* cuda_stream, const int32_t* h_ve
 }
 
 // ------------------------------------------------------------------------------------------
+// occupancy: k^3 sub-samples per voxel folded from the k-times finer bit grid (include/vox.h).  HBM bound:
+// one thread reads the k*k fine words above one run of 32/k coarse voxels and writes 32/k bytes.
+// ------------------------------------------------------------------------------------------
+template <int K>
+__global__ void __launch_bounds__(256) k_occupancy(const u32* __restrict__ fine, int nx, int ny, int nz, int batch,
+                                                   unsigned char* __restrict__ out) {
+    constexpr int PER = 32 / K;                 // coarse voxels per fine word
+    const int fw = (nx * K) >> 5;               // fine words per fine row
+    const i64 total = (i64)batch * nz * ny * fw;
+    const i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const int w = (int)(i % fw);
+    i64 rest = i / fw;
+    const int y = (int)(rest % ny);
+    rest /= ny;
+    const int z = (int)(rest % nz);
+    const i64 m = rest / nz;
+    u32 cnt[PER];
+#pragma unroll
+    for (int j = 0; j < PER; ++j) cnt[j] = 0;
+    const i64 fny = (i64)ny * K, fnz = (i64)nz * K;
+#pragma unroll
+    for (int dz = 0; dz < K; ++dz)
+#pragma unroll
+        for (int dy = 0; dy < K; ++dy) {
+            const u32 v = __ldg(fine + ((m * fnz + (i64)z * K + dz) * fny + (i64)y * K + dy) * fw + w);
+#pragma unroll
+            for (int j = 0; j < PER; ++j) cnt[j] += __popc((v >> (j * K)) & ((1u << K) - 1u));
+        }
+    unsigned char* dst = out + ((m * nz + z) * (i64)ny + y) * nx + (i64)w * PER;
+    u32 packed[PER / 4];
+#pragma unroll
+    for (int q = 0; q < PER / 4; ++q)
+        packed[q] = cnt[4 * q] | (cnt[4 * q + 1] << 8) | (cnt[4 * q + 2] << 16) | (cnt[4 * q + 3] << 24);
+    if (PER == 16) *reinterpret_cast<uint4*>(dst) = make_uint4(packed[0], packed[1], packed[2], packed[3]);
+    else *reinterpret_cast<uint2*>(dst) = make_uint2(packed[0], packed[1 % (PER / 4)]);
+}
+
+extern "C" int vox_occupancy(void* cuda_stream, const uint32_t* d_bits_fine, int nx, int ny, int nz, int batch, int k,
+                             uint8_t* d_counts_out) {
+    if (!d_bits_fine || !d_counts_out || nx <= 0 || ny <= 0 || nz <= 0 || batch < 1) return VOX_EINVAL;
+    if ((k != 2 && k != 4) || ((i64)nx * k) % 32 != 0) return VOX_EINVAL;
+    if (((uintptr_t)d_counts_out & 15) != 0) return VOX_EINVAL;  // vector stores
+    const i64 total = (i64)batch * nz * ny * ((nx * k) >> 5);
+    if (total > 0x7FFFFFFFll * 256) return VOX_ERANGE;
+    const unsigned blocks = (unsigned)((total + 255) / 256);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (k == 2) k_occupancy<2><<<blocks, 256, 0, st>>>(d_bits_fine, nx, ny, nz, batch, d_counts_out);
+    else k_occupancy<4><<<blocks, 256, 0, st>>>(d_bits_fine, nx, ny, nz, batch, d_counts_out);
+    return cudaGetLastError() == cudaSuccess ? VOX_OK : VOX_ECUDA;
+}
+
+// ------------------------------------------------------------------------------------------
 // vox_pipe: transfer-overlapped pipeline over a stream of host meshes (include/vox.h)
 // ------------------------------------------------------------------------------------------
 enum { PIPE_MAX_DEPTH = 8 };
