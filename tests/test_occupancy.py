@@ -104,3 +104,19 @@ def test_gpu_occupancy_argument_checks():
     assert lib.vox_occupancy(None, p, 16, 4, 4, 1, 3, p) == -1      # k
     assert lib.vox_occupancy(None, p, 12, 4, 4, 1, 2, p) == -1      # (k*nx) % 32
     assert lib.vox_occupancy(None, None, 16, 4, 4, 1, 2, p) == -1
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("nx,ny,nz,batch,k", [(16, 5, 3, 2, 4), (48, 7, 2, 1, 2), (64, 3, 5, 3, 2), (32, 4, 4, 1, 4),
+                                               (8, 2, 2, 1, 4)])
+def test_gpu_occupancy_on_random_bits(nx, ny, nz, batch, k):
+    """Scalar and 16-byte-vector variants, odd row counts, batches: random fine bit grids straight into the fold."""
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    rng = np.random.default_rng(nx * 131 + ny * 17 + nz + k)
+    fine = rng.integers(0, 2**32, (batch, k * nz, k * ny, k * nx // 32), dtype=np.uint64).astype(np.uint32)
+    fine[rng.random(fine.shape) < 0.2] = 0xFFFFFFFF
+    got = pkg.occupancy(torch.from_numpy(fine.view(np.int32)).cuda(), (nx, ny, nz), k, batch=batch).cpu().numpy()
+    assert np.array_equal(got, occupancy(fine, k))
