@@ -478,8 +478,8 @@ def run_b200(args):
             occ = {"k": 2, "coarse_grid": list(cgrid), "ms": oms, "bytes": obytes, "bound": "hbm",
                    "achieved_gbs": obytes / (oms * 1e-3) / 1e9, "peak_gbs": hbm_peak,
                    "frac": obytes / (oms * 1e-3) / 1e9 / hbm_peak,
-                   "note": "repeated on the same 268 MB (> 126 MB L2); sum(counts) == popcount: "
-                           + str(int(counts.sum(dtype=torch.int64)) == popcount)}
+                   "note": f"20 launches back to back on the same {obytes / 1e6:.0f} MB (L2 holds 126 MB); "
+                           f"sum(counts) == popcount: {int(counts.sum(dtype=torch.int64)) == popcount}"}
 
         cpu = None
         if not args.no_cpu_baseline:

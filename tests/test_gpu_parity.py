@@ -160,7 +160,8 @@ def test_stale_output_is_overwritten():
     [((32, 24, 40), (32 * 6, 24 * 10, 40 * 14)),     # pitches 6,10,14: gcd 2
      ((64, 20, 12), (64 * 6, 20 * 12, 12 * 18)),     # pitches 6,12,18: gcd 6 (not a power of two)
      ((32, 40, 24), (32 * 2048, 40 * 512, 24 * 4096)),
-     ((96, 33, 7), (96 * 4, 33 * 4, 7 * 4))],
+     ((96, 33, 7), (96 * 4, 33 * 4, 7 * 4)),
+     ((4096, 40, 24), (4096 * 16, 40 * 512, 24 * 1024))],   # 128 tiles along x
 )
 def test_ragged_anisotropic_grids(grid, extent):
     rng = np.random.default_rng(sum(grid))
