@@ -582,7 +582,7 @@ __global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__
 //   mx_G == 0:          r' = 64*G + 63, mx = 0 (hi) -> gates the row only (see span_plane)
 // b = floor of the real crossing r/|mx|.  A fixed-point reciprocal PROPOSES c0 = floor(r*inv/2^32), which is
 // B or B+1 for r >= 0 (see span_bound); the INTEGER value Q(c0) decides: b = c0 if Q(c0) >= 0 else c0-1.
-// No floating point at all.  Planes are stored scaled by 2 (by 4 when |mx| = 1) so that |mx| >= 4 and the
+// No floating point at all.  Planes are stored scaled by 4 so that |mx| >= 4 and the
 // reciprocal fits int32; all stored Q(x), x in [-1,32], and r +- mx fit int32 (checked in int64 at setup).
 // ------------------------------------------------------------------------------------------
 enum { SREC_W = 40, KIND_SPAN = 0, IMG_SKEW = 11, R_BOX = 38, R_INFO = 39 };  // record stride 40 words: int4-aligned
@@ -608,11 +608,14 @@ __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, i
     ok = ok && ((u64)(g64 + (1ll << 30)) < (1ull << 31));                          // |g0| <= 2^30
     int g0 = (int)g64;
     if (mx > 0) { mx = (int)(0u - (u32)mx); my = (int)(0u - (u32)my); mz = (int)(0u - (u32)mz); g0 = ~g0; }  // lo-type: Q = -G - 1
-    // scale: 2 (4 when |mx| == 1) so that the reciprocal ceil(2^32 / |mx|) fits int32; a plane with mx == 0 does
+    // scale: 4, so that |mx| >= 4 and the reciprocal ceil(2^32 / |mx|) fits int32; a plane with mx == 0 does
     // not depend on x and only gates the row: stored as r' = 64*G + 63 with inv = 2^31 - 1, for which span_bound
     // gives c0 = floor(r'/2 - r'/2^32) >= 31 when r' >= 63 (G >= 0: not binding, x1' <= 31) and b = c0 - 1 <= -2
     // when r' <= -1 (G < 0: empty row).
-    const int sh = (mx == 0) ? 6 : ((mx == -1) ? 2 : 1);
+    // (every x-dependent plane is scaled by 4, not "2, or 4 when |mx| == 1": ptxas 12.9 at -O1 and above folds the
+    //  test `mx == -1` on the negated absolute value to false -- SASS keeps only the cases 1 and 6 -- which the
+    //  parity suite caught twice)
+    const int sh = (mx == 0) ? 6 : 2;
     // every row value r of the box and r +- 2*mx (span_bound's product and check) must fit int32 after scaling
     u64 acc = (u64)(u32)abs(g0) + 2ull * (0u - (u32)mx);
     acc += (u64)(u32)wy * (u32)abs(my);

@@ -431,3 +431,67 @@ def test_planes_with_unit_and_zero_x_normal_component():
         assert_same(gpu_voxelize(m, tile=tile), exp, f"unit nx tile={tile}")
     m2 = Mesh("unit_nx_fine", m.verts, m.tets, (256, 256, 256))
     assert_same(gpu_voxelize(m2), cpu_voxelize(m2), "unit nx 256^3")
+
+
+# ------------------------------------------------------------------ randomized differential test
+def _random_job(seed):
+    """A random grid (anisotropic pitches, ragged dims), a random batch and a soup of tets of every size class:
+    sub-voxel slivers, few-voxel tets, tile-sized tets, grid-spanning giants, degenerate and axis-aligned ones."""
+    rng = np.random.default_rng(seed)
+    nx = 32 * int(rng.integers(1, 5))
+    ny, nz = int(rng.integers(1, 71)), int(rng.integers(1, 71))
+    pitch = [2 * int(rng.integers(1, 600)) for _ in range(3)]
+    if seed % 3 == 0:
+        pitch = [int(2 ** rng.integers(1, 11))] * 3          # the common case: equal power-of-two pitches
+    extent = (nx * pitch[0], ny * pitch[1], nz * pitch[2])
+    if max(extent) > (1 << 20):
+        return None
+    batch = int(rng.integers(1, 4))
+    ext = np.array(extent)
+    verts, tets, offsets = [], [], [0]
+    for _ in range(batch):
+        n_t = int(rng.integers(0, 120))
+        for _t in range(n_t):
+            kind = rng.integers(0, 6)
+            c = rng.integers(0, ext + 1)
+            size = [np.array(pitch) // 2 + 1, np.array(pitch) * 3, np.array(pitch) * 12, ext // 2 + 1, ext + 1,
+                    np.array(pitch) * 3][kind]
+            pts = c + rng.integers(-size, size + 1, (4, 3))
+            if kind == 5:                                      # axis-aligned faces / samples on faces
+                pts = (pts // (np.array(pitch) // 2 + 1)) * (np.array(pitch) // 2 + 1)
+            if rng.random() < 0.05:
+                pts[3] = pts[rng.integers(0, 3)]               # degenerate: repeated vertex
+            pts = np.clip(pts, 0, ext)
+            base = len(verts)
+            verts += pts.tolist()
+            tets.append([base, base + 1, base + 2, base + 3])
+        offsets.append(len(tets))
+    if not verts:
+        verts = [[0, 0, 0]] * 4
+    v = np.array(verts, dtype=np.int32).reshape(-1, 3)
+    t = np.array(tets, dtype=np.int32).reshape(-1, 4)
+    m = Mesh(f"fuzz{seed}", v, t, (nx, ny, nz), extent)
+    if batch > 1:
+        m = Mesh(f"fuzz{seed}", v, t, (nx, ny, nz), extent, tet_offsets=np.array(offsets, dtype=np.int64))
+    tile = [None, (4, 4), (8, 32), (32, 32), (16, 8)][int(rng.integers(0, 5))]
+    return m, tile
+
+
+@pytest.mark.parametrize("block", range(6))
+def test_randomized_jobs_match_oracle(block):
+    from oracle import sparse
+
+    done = 0
+    for seed in range(1000 + 12 * block, 1000 + 12 * (block + 1)):
+        job = _random_job(seed)
+        if job is None:
+            continue
+        m, tile = job
+        exp = cpu_voxelize(m)
+        got = gpu_voxelize(m, tile=tile)
+        assert_same(got, exp, f"fuzz seed {seed} grid {m.grid} extent {m.extent} batch {m.batch} tile {tile}")
+        if seed % 4 == 0:
+            table, payload, ts, st = _gpu_sparse(m, tile)
+            assert sparse.check_table(table, payload, exp, ts["ty"], ts["tz"]) == st["mixed_tiles"], f"seed {seed}"
+        done += 1
+    assert done >= 6
