@@ -495,3 +495,30 @@ def test_randomized_jobs_match_oracle(block):
             assert sparse.check_table(table, payload, exp, ts["ty"], ts["tz"]) == st["mixed_tiles"], f"seed {seed}"
         done += 1
     assert done >= 6
+
+
+def test_randomized_magnitudes_straddle_the_int32_limit():
+    """Random tets of 2^4..2^13.5 lattice units on lattices of extent 2^14..2^20: about half of the (tet, tile)
+    pairs fit the int32 span path and half take the int64 large path, so the hand-over bound is exercised from
+    both sides."""
+    import paper_2106_01326_b200 as pkg
+
+    large = pairs = 0
+    for seed in range(80):
+        rng = np.random.default_rng(seed)
+        n = int(rng.choice([32, 64, 128, 256]))
+        Ex = 1 << int(rng.integers(14, 21))
+        verts, tets = [], []
+        for _ in range(int(rng.integers(5, 60))):
+            size = int(2 ** rng.uniform(4, 13.5))
+            c = rng.integers(0, Ex + 1, 3)
+            pts = np.clip(c + rng.integers(-size // 2, size // 2 + 1, (4, 3)), 0, Ex)
+            b = len(verts)
+            verts += pts.tolist()
+            tets.append([b, b + 1, b + 2, b + 3])
+        m = Mesh(f"mag{seed}", np.array(verts, dtype=np.int32), np.array(tets, dtype=np.int32), (n, n, n), (Ex,) * 3)
+        tile = [None, (8, 8), (32, 32)][int(rng.integers(0, 3))]
+        assert_same(gpu_voxelize(m, tile=tile), cpu_voxelize(m), f"magnitude seed {seed} n {n} E {Ex} tile {tile}")
+        large += pkg.voxelize.last_status["large_pairs"]
+        pairs += pkg.voxelize.last_status["pairs"]
+    assert 0.2 * pairs < large < 0.8 * pairs
