@@ -653,6 +653,17 @@ __device__ __noinline__ void large_record(const Params& p, u32 t, int X0, int Y0
     rec[20] = 0; rec[21] = -2; rec[22] = 1; rec[23] = 1; rec[24] = (int)img_saddr; rec[25] = 0;
 }
 
+// b = max{x in [0,31] : q0 - a*x >= 0}, or -1 if there is none (a > 0).  A float quotient PROPOSES (its error is
+// far below 1 for quotients up to 32), the exact int64 value decides; quotients beyond 31 saturate.
+__device__ __forceinline__ int span64_bound(i64 q0, i64 a) {
+    if (q0 < 0) return -1;
+    int c = (int)fminf(__ll2float_rn(q0) / __ll2float_rn(a), 31.0f);
+    const i64 v = q0 - a * c;
+    if (v < 0) c -= 1;
+    else if (c < 31 && v - a >= 0) c += 1;
+    return c;
+}
+
 // the same, with the int64 planes already in the pair's shared-memory record (large_record)
 __device__ __noinline__ void raster_large_rec(const int* rec, u32* img, int lane, int img_stride) {
     Planes P;
@@ -687,6 +698,26 @@ __device__ __noinline__ void raster_large_rec(const int* rec, u32* img, int lane
         }
         return;
     }
+    const int nrows = ny * (z1 - z0 + 1);
+    if (nrows > 5) {
+        // many rows: lanes = rows, each lane finds its row's span from four exact int64 bounds (span64_bound)
+        for (int r = lane; r < nrows; r += 32) {
+            const int zz = r / ny;
+            const int y = y0 + r - zz * ny, z = z0 + zz;
+            int lower = x0 - 1, upper = x1;  // solid x in (lower, upper]
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const i64 G0 = P.g0[k] + P.my[k] * y + P.mz[k] * z;  // G at x = 0 of this row
+                if (P.mx[k] > 0) lower = max(lower, span64_bound(-G0 - 1, P.mx[k]));          // G(x) >= 0 <=> x >= b + 1
+                else if (P.mx[k] < 0) upper = min(upper, span64_bound(G0, -P.mx[k]));         // G(x) >= 0 <=> x <= b
+                else if (G0 < 0) upper = -2;                                                   // x-independent plane
+            }
+            const int n = upper - lower;
+            if (n > 0) atomicOr(img + z * img_stride + y, (0xFFFFFFFFu >> (32 - n)) << (lower + 1));
+        }
+        return;
+    }
+    // few rows: lanes = the 32 x positions of a row word, __ballot_sync forms the word
     i64 c0 = P.g0[0] + P.mx[0] * lane, c1 = P.g0[1] + P.mx[1] * lane;
     i64 c2 = P.g0[2] + P.mx[2] * lane, c3 = P.g0[3] + P.mx[3] * lane;
     for (int z = z0; z <= z1; ++z) {
