@@ -69,7 +69,10 @@ enum { TM_EV = 5 };  // before memset/K1, after K1, after K2, after K3, after K4
 enum { HDR_WORDS = 64 };
 // header words
 enum { H_TOTAL = 0, H_OVERFLOW = 1, H_CULLED = 2, H_LARGE = 3, H_NONEMPTY = 4, H_BAD = 5, H_TOTAL_HI = 6,
-       H_MIXED = 7, H_FULL = 8, H_PAYLOAD_OVERFLOW = 9 };
+       H_MIXED = 7, H_FULL = 8, H_PAYLOAD_OVERFLOW = 9, H_NBIG = 10 };
+// tets whose tile range exceeds BIG_TILES are not binned by their own thread: K1 lists them and K2's CTA
+// (1024 threads) counts and scatters their tiles
+enum { BIG_TILES = 64, BIG_CAP = 4096, RANGE_BIG = 0x40000000 };
 // sparse tile table codes (include/vox.h)
 #define TILE_EMPTY 0u
 #define TILE_FULL 0xFFFFFFFFu
@@ -78,7 +81,7 @@ enum { H_TOTAL = 0, H_OVERFLOW = 1, H_CULLED = 2, H_LARGE = 3, H_NONEMPTY = 4, H
 static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct WsLayout {
-    size_t hdr, counts, cursor, range, list, fixed_end;
+    size_t hdr, counts, cursor, big, range, list, fixed_end;
 };
 static WsLayout ws_layout(const Params& p) {
     WsLayout L;
@@ -89,6 +92,8 @@ static WsLayout ws_layout(const Params& p) {
     o = align256(o + ((size_t)p.NB + 1) * 4);
     L.cursor = o;
     o = align256(o + ((size_t)p.NB + 1) * 4);
+    L.big = o;
+    o = align256(o + (size_t)BIG_CAP * 4);
     L.range = o;
     o = align256(o + (size_t)(p.T > 0 ? p.T : 1) * 8);
     L.list = o;
@@ -163,9 +168,9 @@ __device__ __forceinline__ int mesh_of(const Params& p, i64 t) {
 #define RANGE_CULLED 0xFFFFFFFFu
 
 __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ range, u32* __restrict__ counts,
-                                                u32* __restrict__ hdr) {
+                                                u32* __restrict__ hdr, u32* __restrict__ big) {
     i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-    bool live = false;
+    bool live = false, handed = false;
     uint2 r = make_uint2(RANGE_CULLED, 0u);
     int m = 0;
     int b0x = 0, b1x = -1, b0y = 0, b1y = -1, b0z = 0, b1z = -1;
@@ -183,6 +188,14 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
             r.x = (u32)b0x | ((u32)b0y << 10) | ((u32)b0z << 20);
             r.y = (u32)b1x | ((u32)b1y << 10) | ((u32)b1z << 20);
             m = mesh_of(p, t);
+            if ((b1x - b0x + 1) * (b1y - b0y + 1) * (b1z - b0z + 1) > BIG_TILES) {  // oversized: hand over to K2
+                const u32 slot = atomicAdd(hdr + H_NBIG, 1u);
+                if (slot < (u32)BIG_CAP) {
+                    big[slot] = (u32)t;
+                    r.x |= RANGE_BIG;
+                    handed = true;
+                }
+            }
         }
         range[t] = r;
     }
@@ -190,6 +203,7 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
     if ((threadIdx.x & 31) == 0 && dead) atomicAdd(hdr + H_CULLED, __popc(dead));
     // warp-aggregated histogram: in step k every live lane names the k-th tile of its range; lanes
     // naming the same tile (neighbouring tets mostly do) are merged into one atomic
+    live = live && !handed;
     int cx = b0x, cy = b0y, cz = b0z;
     const int lane = threadIdx.x & 31;
     for (;;) {
@@ -214,8 +228,37 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
 // K2: exclusive scan of counts[0..NB) (single CTA, 4096 counters per pass; NB is at most a few 10^5)
 // counts[b] <- offset, counts[NB] <- total, cursor[b] <- offset
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024) k2_scan(u32 NB, u32* __restrict__ counts, u32* __restrict__ cursor,
-                                                u32* __restrict__ hdr) {
+// tile b of the idx-th tile of a packed range
+__device__ __forceinline__ u32 range_tile(const Params& p, uint2 r, int m, u32 idx) {
+    const u32 b0x = r.x & 1023, b0y = (r.x >> 10) & 1023, b0z = (r.x >> 20) & 1023;
+    const u32 wx = (r.y & 1023) - b0x + 1, wy = ((r.y >> 10) & 1023) - b0y + 1;
+    const u32 dx = idx % wx, rest = idx / wx;
+    const u32 dy = rest % wy, dz = rest / wy;
+    return ((((u32)m * p.nbz + b0z + dz) * p.nby + b0y + dy) * p.nbx) + b0x + dx;
+}
+__device__ __forceinline__ u32 range_tiles(uint2 r) {
+    const u32 wx = (r.y & 1023) - (r.x & 1023) + 1, wy = ((r.y >> 10) & 1023) - ((r.x >> 10) & 1023) + 1;
+    const u32 wz = ((r.y >> 20) & 1023) - ((r.x >> 20) & 1023) + 1;
+    return wx * wy * wz;
+}
+
+__global__ void __launch_bounds__(1024) k2_scan(Params p, const uint2* __restrict__ range, const u32* __restrict__ big,
+                                                u32* __restrict__ list, u32* __restrict__ counts,
+                                                u32* __restrict__ cursor, u32* __restrict__ hdr, int scatter_big) {
+    const u32 NB = p.NB;
+    // oversized tets (K1 listed them): the whole CTA counts their tiles, 1024 at a time
+    const u32 nbig = min(hdr[H_NBIG], (u32)BIG_CAP);
+    for (u32 e = 0; e < nbig; ++e) {
+        const u32 t = big[e];
+        const uint2 r = range[t];
+        const int m = mesh_of(p, t);
+        const u32 n = range_tiles(r);
+        for (u32 idx = threadIdx.x; idx < n; idx += 1024u) atomicAdd(counts + range_tile(p, r, m, idx), 1u);
+    }
+    if (nbig) {
+        __threadfence();
+        __syncthreads();
+    }
     // chunks of 4096 counters: one coalesced uint4 per thread, warp shuffle scan, 32 warp partials
     // scanned by warp 0, running carry in 64 bits (a total above 2^32 raises the overflow flag)
     __shared__ u64 s_warp[32];
@@ -227,12 +270,12 @@ __global__ void __launch_bounds__(1024) k2_scan(u32 NB, u32* __restrict__ counts
     u32 ne = 0;
     auto load4 = [&](u32 i) {
         uint4 c = make_uint4(0u, 0u, 0u, 0u);
-        if (i + 3 < NB && vec_ok) c = *reinterpret_cast<const uint4*>(counts + i);
+        if (i + 3 < NB && vec_ok) c = __ldcg(reinterpret_cast<const uint4*>(counts + i));
         else {
-            if (i < NB) c.x = counts[i];
-            if (i + 1 < NB) c.y = counts[i + 1];
-            if (i + 2 < NB) c.z = counts[i + 2];
-            if (i + 3 < NB) c.w = counts[i + 3];
+            if (i < NB) c.x = __ldcg(counts + i);
+            if (i + 1 < NB) c.y = __ldcg(counts + i + 1);
+            if (i + 2 < NB) c.z = __ldcg(counts + i + 2);
+            if (i + 3 < NB) c.w = __ldcg(counts + i + 3);
         }
         return c;
     };
@@ -295,6 +338,21 @@ __global__ void __launch_bounds__(1024) k2_scan(u32 NB, u32* __restrict__ counts
         for (int k = 0; k < 32; ++k) s += s_ne[k];
         hdr[H_NONEMPTY] = s;
     }
+    if (nbig && scatter_big) {  // scatter the oversized tets (K3 appends the others to the same cursors afterwards)
+        __threadfence();
+        __syncthreads();
+        for (u32 e = 0; e < nbig; ++e) {
+            const u32 t = big[e];
+            const uint2 r = range[t];
+            const int m = mesh_of(p, t);
+            const u32 n = range_tiles(r);
+            for (u32 idx = threadIdx.x; idx < n; idx += 1024u) {
+                const u32 pos = atomicAdd(cursor + range_tile(p, r, m, idx), 1u);
+                if (pos < p.cap) list[pos] = t;
+                else hdr[H_OVERFLOW] = 1;
+            }
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -307,7 +365,7 @@ __global__ void __launch_bounds__(256) k3_scatter(Params p, const uint2* __restr
     int b0x = 0, b0y = 0, b1x = 0, b1y = 0, b1z = 0, cx = 0, cy = 0, cz = 0, m = 0;
     if (t < p.T) {
         const uint2 r = range[t];
-        if (r.x != RANGE_CULLED) {
+        if (r.x != RANGE_CULLED && !(r.x & RANGE_BIG)) {  // (oversized tets were scattered by K2)
             live = true;
             b0x = r.x & 1023; b0y = (r.x >> 10) & 1023; cz = (r.x >> 20) & 1023;
             b1x = r.y & 1023; b1y = (r.y >> 10) & 1023; b1z = (r.y >> 20) & 1023;
@@ -1388,22 +1446,24 @@ extern "C" size_t vox_workspace_bytes(const vox_ctx* ctx) {
     return ws_layout(p).fixed_end + align256((size_t)pairs * 4);
 }
 
-static int enqueue_count_scan(vox_ctx* ctx, cudaStream_t st, char* ws, cudaEvent_t* ev) {
+// with_list: the pair list exists (vox_run); vox_plan only counts
+static int enqueue_count_scan(vox_ctx* ctx, cudaStream_t st, char* ws, cudaEvent_t* ev, bool with_list) {
     Params& p = ctx->p;
     WsLayout L = ws_layout(p);
     u32* hdr = (u32*)(ws + L.hdr);
     u32* counts = (u32*)(ws + L.counts);
     u32* cursor = (u32*)(ws + L.cursor);
+    u32* big = (u32*)(ws + L.big);
     uint2* range = (uint2*)(ws + L.range);
     if (ev) CK(cudaEventRecord(ev[0], st));
     // header and counts are adjacent: one memset
     CK(cudaMemsetAsync(ws + L.hdr, 0, L.cursor - L.hdr, st));
     if (p.T > 0) {
         unsigned blocks = (unsigned)((p.T + 255) / 256);
-        k1_count<<<blocks, 256, 0, st>>>(p, range, counts, hdr);
+        k1_count<<<blocks, 256, 0, st>>>(p, range, counts, hdr, big);
     }
     if (ev) CK(cudaEventRecord(ev[1], st));
-    k2_scan<<<1, 1024, 0, st>>>(p.NB, counts, cursor, hdr);
+    k2_scan<<<1, 1024, 0, st>>>(p, range, big, (u32*)(ws + L.list), counts, cursor, hdr, with_list ? 1 : 0);
     CK(cudaGetLastError());
     if (ev) CK(cudaEventRecord(ev[2], st));
     return VOX_OK;
@@ -1415,7 +1475,7 @@ extern "C" int vox_plan(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size
     WsLayout L = ws_layout(ctx->p);
     if (ws_bytes < L.fixed_end) return VOX_EWORKSPACE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int rc = enqueue_count_scan(ctx, st, (char*)d_workspace, NULL);
+    int rc = enqueue_count_scan(ctx, st, (char*)d_workspace, NULL, false);
     if (rc) return rc;
     u32 h[HDR_WORDS];
     CK(cudaMemcpyAsync(h, (char*)d_workspace + L.hdr, sizeof(h), cudaMemcpyDeviceToHost, st));
@@ -1475,7 +1535,7 @@ static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t w
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char* ws = (char*)d_workspace;
     cudaEvent_t* ev = ctx->tm_ev ? ctx->tm_ev + (size_t)(ctx->tm_next % ctx->tm_slots) * TM_EV : NULL;
-    int rc = enqueue_count_scan(ctx, st, ws, ev);
+    int rc = enqueue_count_scan(ctx, st, ws, ev, true);
     if (rc) return rc;
     u32* hdr = (u32*)(ws + L.hdr);
     u32* counts = (u32*)(ws + L.counts);

@@ -522,3 +522,24 @@ def test_randomized_magnitudes_straddle_the_int32_limit():
         large += pkg.voxelize.last_status["large_pairs"]
         pairs += pkg.voxelize.last_status["pairs"]
     assert 0.2 * pairs < large < 0.8 * pairs
+
+
+def test_more_oversized_tets_than_the_handover_list_holds():
+    """Tets whose tile range exceeds 64 tiles are handed from K1 to K2's CTA through a 4096-entry list; with 5000 of
+    them the rest falls back to the per-thread walk.  Both routes in one mesh, plus small tets."""
+    import paper_2106_01326_b200 as pkg
+
+    rng = np.random.default_rng(4096)
+    verts, tets = [], []
+    for i in range(5200):
+        size = 36000 if i < 5000 else 900                  # ~70 voxels of 512 lattice units, or ~2 voxels
+        c = rng.integers(0, E + 1, 3)
+        pts = np.clip(c + rng.integers(-size // 2, size // 2 + 1, (4, 3)), 0, E)
+        b = len(verts)
+        verts += pts.tolist()
+        tets.append([b, b + 1, b + 2, b + 3])
+    m = Mesh("oversized", np.array(verts, dtype=np.int32), np.array(tets, dtype=np.int32), (128, 128, 128))
+    exp = cpu_voxelize(m)
+    assert_same(gpu_voxelize(m, tile=(8, 8)), exp, "oversized tile=(8,8)")
+    assert pkg.voxelize.last_status["pairs"] > 64 * 4096
+    assert_same(gpu_voxelize(m), exp, "oversized auto tile")
