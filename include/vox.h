@@ -79,6 +79,16 @@ int vox_set_variant(vox_ctx* ctx, int variant);
 int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const int32_t* d_tets, int64_t T,
              const int64_t* d_tet_offsets);
 
+/* Lattice input ("combining the background grid insertion method ... with the grid method for
+ * voxelization sampling").  When the tet mesh IS a (jittered, carved) background lattice there is no
+ * need for a tet array: d_verts int32[(cx+1)*(cy+1)*(cz+1)][3] holds the lattice vertices, vertex (i,j,k) at index
+ * (i*(cy+1) + j)*(cz+1) + k; cell (i,j,k), index c = (i*cy + j)*cz + k, is split into the 6 Kuhn tets, tet q
+ * walking from the cell's low corner along the axes of the q-th permutation of (x,y,z) in lexicographic order
+ * (xyz, xzy, yxz, yzx, zxy, zyx); bit q of d_keep[c] says whether tet q is present.  Equivalent to vox_tets with
+ * the 6*cx*cy*cz tets written out (absent ones dropped); batch must be 1.  vox_status counts only present tets
+ * as culled. */
+int vox_lattice(vox_ctx* ctx, const int32_t* d_verts, int cx, int cy, int cz, const uint8_t* d_keep);
+
 /* batch * nz * ny * (nx/32) */
 size_t vox_grid_words(const vox_ctx* ctx);
 
@@ -205,6 +215,11 @@ int vox_pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int
 int vox_pipe_submit_sparse(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,
                            const int64_t* h_tet_offsets, uint32_t* h_table, uint32_t* h_payload,
                            int64_t payload_capacity_tiles, int64_t* ticket_out);
+/* Lattice input through the pipe (vox_lattice): h_verts int32[(cx+1)(cy+1)(cz+1)][3] and h_keep uint8[cx*cy*cz],
+ * pinned.  payload_capacity_tiles < 0: dense (h_out = the grid); otherwise sparse (h_out = tile table, h_payload as
+ * in vox_pipe_submit_sparse).  The pipe must have been created with max_T >= 6*cx*cy*cz. */
+int vox_pipe_submit_lattice(vox_pipe* pipe, const int32_t* h_verts, int cx, int cy, int cz, const uint8_t* h_keep,
+                            uint32_t* h_out, uint32_t* h_payload, int64_t payload_capacity_tiles, int64_t* ticket_out);
 int vox_pipe_wait(vox_pipe* pipe, int64_t ticket, int64_t stats_out[6]);
 int vox_pipe_tile_shape(const vox_pipe* pipe, int out[5]);
 const char* vox_pipe_last_error(const vox_pipe* pipe);

@@ -18,4 +18,5 @@ from .kuhn import (  # noqa: F401
     carve_every_third,
     carve_sphere,
     single_tet_mesh,
+    lattice_form,
 )

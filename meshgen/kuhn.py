@@ -312,6 +312,38 @@ def carve_sphere(m: Mesh, frac: float = 0.4) -> Mesh:
     return Mesh(m.name + "_sphere", m.verts, t, m.grid, m.extent)
 
 
+def lattice_form(m: Mesh, cells) -> np.ndarray:
+    """keep mask uint8[cx*cy*cz] of a (carved) kuhn_mesh job with `cells` = (cx, cy, cz): bit q of cell c is set iff
+    the cell's q-th tet (q = index into the lexicographic permutations of the axes, as kuhn_mesh lists them) is in
+    m.tets.  With m.verts this is the lattice input of include/vox.h ("vox_lattice"); m.tets is the same mesh
+    written out.  Pure index bookkeeping."""
+    assert m.batch == 1
+    cx, cy, cz = (int(c) for c in cells)
+    assert m.V == (cx + 1) * (cy + 1) * (cz + 1)
+    t = m.tets.astype(np.int64)
+    v0 = t[:, 0]
+    k = v0 % (cz + 1)
+    j = (v0 // (cz + 1)) % (cy + 1)
+    i = v0 // ((cz + 1) * (cy + 1))
+    sx, sy = (cy + 1) * (cz + 1), cz + 1  # vertex-id strides of a step along x, y (z: 1)
+
+    def axis(d):
+        return np.where(d == sx, 0, np.where(d == sy, 1, 2))
+
+    a1, a2 = axis(t[:, 1] - t[:, 0]), axis(t[:, 2] - t[:, 1])
+    q = _perm_index(a1, a2)
+    keep = np.zeros(cx * cy * cz, dtype=np.uint8)
+    np.bitwise_or.at(keep, (i * cy + j) * cz + k, (1 << q).astype(np.uint8))
+    return keep
+
+
+def _perm_index(a1, a2):
+    table = np.full((3, 3), -1, dtype=np.int64)
+    for q, perm in enumerate(_PERMS):
+        table[perm[0], perm[1]] = q
+    return table[a1, a2]
+
+
 def single_tet_mesh(a, b, c, d, grid=(32, 32, 32), extent=(E_LATTICE,) * 3) -> Mesh:
     v = np.array([a, b, c, d], dtype=np.int32)
     t = np.array([[0, 1, 2, 3]], dtype=np.int32)

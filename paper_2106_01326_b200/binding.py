@@ -17,7 +17,7 @@ EXPORTS = [
     "vox_pipe_create", "vox_pipe_destroy", "vox_pipe_set_variant", "vox_pipe_set_tile", "vox_pipe_arena_bytes",
     "vox_pipe_bind", "vox_pipe_submit", "vox_pipe_wait", "vox_pipe_last_error",
     "vox_tile_shape", "vox_run_sparse", "vox_sparse_status", "vox_pipe_submit_sparse", "vox_pipe_tile_shape",
-    "vox_pipe_reserve_pairs", "vox_occupancy",
+    "vox_pipe_reserve_pairs", "vox_occupancy", "vox_lattice", "vox_pipe_submit_lattice",
 ]
 
 
@@ -79,6 +79,8 @@ def load_library():
         "vox_pipe_tile_shape": (i32, [vp, ctypes.POINTER(i32)]),
         "vox_pipe_reserve_pairs": (i32, [vp, i64]),
         "vox_occupancy": (i32, [vp, vp, i32, i32, i32, i32, i32, vp]),
+        "vox_lattice": (i32, [vp, vp, i32, i32, i32, vp]),
+        "vox_pipe_submit_lattice": (i32, [vp, vp, i32, i32, i32, vp, vp, vp, i64, ctypes.POINTER(i64)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -178,6 +180,18 @@ class Voxelizer:
         )
         self._keep = (verts, tets, tet_offsets)
         self.T, self.V = T, V
+
+    def set_lattice(self, verts, cells, keep):
+        """vox_lattice: verts int32[(cx+1)(cy+1)(cz+1)][3] and keep uint8[cx*cy*cz] CUDA tensors (include/vox.h)."""
+        torch = _torch_cuda()
+        cx, cy, cz = (int(c) for c in cells)
+        assert verts.is_cuda and verts.dtype == torch.int32 and verts.is_contiguous()
+        assert keep.is_cuda and keep.dtype == torch.uint8 and keep.is_contiguous()
+        assert verts.numel() == 3 * (cx + 1) * (cy + 1) * (cz + 1) and keep.numel() == cx * cy * cz
+        self._ck(self._lib.vox_lattice(self._ctx, ctypes.c_void_p(verts.data_ptr()), cx, cy, cz,
+                                       ctypes.c_void_p(keep.data_ptr())), "vox_lattice")
+        self._keep = (verts, keep)
+        self.T, self.V = 6 * cx * cy * cz, (cx + 1) * (cy + 1) * (cz + 1)
 
     def alloc_workspace(self, nbytes=None):
         torch = _torch_cuda()
@@ -377,6 +391,26 @@ class Pipe:
             "vox_pipe_submit_sparse",
         )
         self._keep[ticket.value] = (h_verts, h_tets, h_table, h_payload, h_tet_offsets)
+        return int(ticket.value)
+
+    def submit_lattice(self, h_verts, cells, h_keep, h_out, h_payload=None, capacity_tiles=-1):
+        """vox_pipe_submit_lattice: lattice vertices + keep mask in (pinned); dense grid out (capacity_tiles < 0)
+        or tile table + payload (sparse)."""
+        bufs = (h_verts, h_keep, h_out) + ((h_payload,) if h_payload is not None else ())
+        for t in bufs:
+            assert not t.is_cuda and t.is_contiguous() and (t.numel() == 0 or t.is_pinned()), \
+                "pipe buffers must be pinned CPU tensors"
+        cx, cy, cz = (int(c) for c in cells)
+        assert h_verts.numel() == 3 * (cx + 1) * (cy + 1) * (cz + 1) and h_keep.numel() == cx * cy * cz
+        ticket = ctypes.c_int64(-1)
+        self._ck(
+            self._lib.vox_pipe_submit_lattice(self._p, ctypes.c_void_p(h_verts.data_ptr()), cx, cy, cz,
+                                              ctypes.c_void_p(h_keep.data_ptr()), ctypes.c_void_p(h_out.data_ptr()),
+                                              ctypes.c_void_p(h_payload.data_ptr()) if h_payload is not None else None,
+                                              int(capacity_tiles), ctypes.byref(ticket)),
+            "vox_pipe_submit_lattice",
+        )
+        self._keep[ticket.value] = bufs
         return int(ticket.value)
 
     def wait(self, ticket):

@@ -29,6 +29,8 @@ struct Params {
     const int32_t* verts;
     const int4* tets;
     const i64* off;  // device, [batch+1] or NULL
+    const unsigned char* keep;  // lattice input (vox_lattice): bit q of keep[cell] = tet q of the cell is present
+    int lcx, lcy, lcz;          // cells per axis of the lattice input; lcx == 0: explicit tets
     i64 T;
     i64 V;
     int batch;
@@ -123,8 +125,26 @@ struct Tet {
     int ax, ay, az, bx, by, bz, cx, cy, cz, dx, dy, dz;
 };
 
+// Lattice input (include/vox.h "vox_lattice"): tet t = 6*cell + q of cell (i,j,k) walks from the cell's low corner
+// along the axes of the q-th permutation of (x,y,z) in lexicographic order; vertex id = (i*(cy+1) + j)*(cz+1) + k.
+__device__ __forceinline__ int4 lattice_ids(const Params& p, i64 t) {
+    const int q = (int)(t % 6);
+    i64 c = t / 6;
+    const int k = (int)(c % p.lcz);
+    c /= p.lcz;
+    const int j = (int)(c % p.lcy);
+    const int i = (int)(c / p.lcy);
+    const int sz = 1, sy = p.lcz + 1, sx = (p.lcy + 1) * (p.lcz + 1);
+    const int v0 = (i * (p.lcy + 1) + j) * (p.lcz + 1) + k;
+    // permutations of (x,y,z), lexicographic: xyz xzy yxz yzx zxy zyx
+    const int a1 = (q < 2) ? sx : (q < 4) ? sy : sz;
+    const int a3 = (q == 3 || q == 5) ? sx : (q == 1 || q == 4) ? sy : sz;
+    const int a2 = sx + sy + sz - a1 - a3;
+    return make_int4(v0, v0 + a1, v0 + a1 + a2, v0 + a1 + a2 + a3);
+}
+
 __device__ __forceinline__ Tet load_tet(const Params& p, i64 t) {
-    int4 id = __ldg(p.tets + t);
+    const int4 id = p.lcx ? lattice_ids(p, t) : __ldg(p.tets + t);
     const int32_t* v = p.verts;
     Tet q;
     q.ax = __ldg(v + 3 * (i64)id.x); q.ay = __ldg(v + 3 * (i64)id.x + 1); q.az = __ldg(v + 3 * (i64)id.x + 2);
@@ -174,7 +194,9 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
     uint2 r = make_uint2(RANGE_CULLED, 0u);
     int m = 0;
     int b0x = 0, b1x = -1, b0y = 0, b1y = -1, b0z = 0, b1z = -1;
-    if (t < p.T) {
+    const bool present = (t < p.T) && (!p.lcx || ((__ldg(p.keep + t / 6) >> (int)(t % 6)) & 1));
+    if (t < p.T && !present) range[t] = r;  // lattice input: the cell does not keep this tet
+    if (present) {
         Tet q = load_tet(p, t);
         int x0, x1, y0, y1, z0, z1;
         axis_range(q.ax, q.bx, q.cx, q.dx, p.hx, p.qx, p.nx, x0, x1);
@@ -199,7 +221,7 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
         }
         range[t] = r;
     }
-    unsigned dead = __ballot_sync(0xFFFFFFFFu, (t < p.T) && !live);
+    unsigned dead = __ballot_sync(0xFFFFFFFFu, present && !live);
     if ((threadIdx.x & 31) == 0 && dead) atomicAdd(hdr + H_CULLED, __popc(dead));
     // warp-aggregated histogram: in step k every live lane names the k-th tile of its range; lanes
     // naming the same tile (neighbouring tets mostly do) are merged into one atomic
@@ -1232,7 +1254,7 @@ __global__ void k_validate(Params p, u32* hdr) {
         int x = p.verts[3 * i], y = p.verts[3 * i + 1], z = p.verts[3 * i + 2];
         bad = bad || x < 0 || x > p.ex || y < 0 || y > p.ey || z < 0 || z > p.ez;
     }
-    if (i < p.T) {
+    if (i < p.T && !p.lcx) {
         int4 id = p.tets[i];
         bad = bad || id.x < 0 || id.x >= p.V || id.y < 0 || id.y >= p.V || id.z < 0 || id.z >= p.V || id.w < 0 || id.w >= p.V;
     }
@@ -1421,7 +1443,28 @@ extern "C" int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const i
     ctx->p.V = V;
     ctx->p.T = T;
     ctx->p.off = (ctx->p.batch > 1) ? (const i64*)d_tet_offsets : NULL;
+    ctx->p.keep = NULL;
+    ctx->p.lcx = ctx->p.lcy = ctx->p.lcz = 0;
     if (!ctx->tile_user) auto_tile(ctx->p, T);
+    ctx->have_tets = true;
+    ctx->pairs_planned = -1;
+    return VOX_OK;
+}
+
+extern "C" int vox_lattice(vox_ctx* ctx, const int32_t* d_verts, int cx, int cy, int cz, const uint8_t* d_keep) {
+    if (!ctx || cx < 1 || cy < 1 || cz < 1 || !d_verts || !d_keep) return VOX_EINVAL;
+    if (ctx->p.batch != 1) return VOX_EINVAL;
+    const i64 cells = (i64)cx * cy * cz, V = (i64)(cx + 1) * (cy + 1) * (cz + 1);
+    if (6 * cells > 0xFFFFFFF0ll || V > 0x7FFFFFFFll) return VOX_ERANGE;
+    Params& p = ctx->p;
+    p.verts = d_verts;
+    p.tets = NULL;
+    p.off = NULL;
+    p.keep = d_keep;
+    p.lcx = cx; p.lcy = cy; p.lcz = cz;
+    p.V = V;
+    p.T = 6 * cells;
+    if (!ctx->tile_user) auto_tile(p, p.T);
     ctx->have_tets = true;
     ctx->pairs_planned = -1;
     return VOX_OK;
@@ -1886,31 +1929,44 @@ static int pipe_finish_slot(vox_pipe* pipe, PipeSlot& s, int64_t stats_out[6]) {
     return (h[H_OVERFLOW] || h[H_PAYLOAD_OVERFLOW]) ? VOX_EWORKSPACE : VOX_OK;
 }
 
+struct LatticeIn { int cx, cy, cz; const uint8_t* h_keep; };  // cx == 0: explicit tets
 static int pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,
-                       const int64_t* h_tet_offsets, uint32_t* h_bits_out, uint32_t* h_payload, int64_t cap_tiles,
-                       int64_t* ticket_out);
+                       const int64_t* h_tet_offsets, LatticeIn lat, uint32_t* h_bits_out, uint32_t* h_payload,
+                       int64_t cap_tiles, int64_t* ticket_out);
 
 extern "C" int vox_pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,
                                const int64_t* h_tet_offsets, uint32_t* h_bits_out, int64_t* ticket_out) {
-    return pipe_submit(pipe, h_verts, V, h_tets, T, h_tet_offsets, h_bits_out, NULL, -1, ticket_out);
+    return pipe_submit(pipe, h_verts, V, h_tets, T, h_tet_offsets, LatticeIn{0, 0, 0, NULL}, h_bits_out, NULL, -1,
+                       ticket_out);
 }
 
 extern "C" int vox_pipe_submit_sparse(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets,
                                       int64_t T, const int64_t* h_tet_offsets, uint32_t* h_table,
                                       uint32_t* h_payload, int64_t payload_capacity_tiles, int64_t* ticket_out) {
     if (payload_capacity_tiles < 0 || (payload_capacity_tiles > 0 && !h_payload)) return VOX_EINVAL;
-    return pipe_submit(pipe, h_verts, V, h_tets, T, h_tet_offsets, h_table, h_payload, payload_capacity_tiles,
+    return pipe_submit(pipe, h_verts, V, h_tets, T, h_tet_offsets, LatticeIn{0, 0, 0, NULL}, h_table, h_payload,
+                       payload_capacity_tiles, ticket_out);
+}
+
+extern "C" int vox_pipe_submit_lattice(vox_pipe* pipe, const int32_t* h_verts, int cx, int cy, int cz,
+                                       const uint8_t* h_keep, uint32_t* h_out, uint32_t* h_payload,
+                                       int64_t payload_capacity_tiles, int64_t* ticket_out) {
+    if (cx < 1 || cy < 1 || cz < 1 || !h_keep || !h_verts) return VOX_EINVAL;
+    if (payload_capacity_tiles > 0 && !h_payload) return VOX_EINVAL;
+    const int64_t cells = (int64_t)cx * cy * cz;
+    return pipe_submit(pipe, h_verts, (int64_t)(cx + 1) * (cy + 1) * (cz + 1), NULL, 6 * cells, NULL,
+                       LatticeIn{cx, cy, cz, h_keep}, h_out, h_payload, payload_capacity_tiles < 0 ? -1 : payload_capacity_tiles,
                        ticket_out);
 }
 
 // cap_tiles < 0: dense (h_bits_out = grid); else sparse (h_bits_out = tile table, h_payload host-mapped)
 static int pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const int32_t* h_tets, int64_t T,
-                       const int64_t* h_tet_offsets, uint32_t* h_bits_out, uint32_t* h_payload, int64_t cap_tiles,
-                       int64_t* ticket_out) {
+                       const int64_t* h_tet_offsets, LatticeIn lat, uint32_t* h_bits_out, uint32_t* h_payload,
+                       int64_t cap_tiles, int64_t* ticket_out) {
     if (!pipe || !h_bits_out || V < 0 || T < 0) return VOX_EINVAL;
     if (!pipe->bound) return VOX_ESTATE;
     if (V > pipe->maxV || T > pipe->maxT) return VOX_ERANGE;
-    if (T > 0 && (!h_verts || !h_tets)) return VOX_EINVAL;
+    if (T > 0 && (!h_verts || (!h_tets && !lat.cx))) return VOX_EINVAL;
     PipeSlot& s = pipe->slot[pipe->next_ticket % pipe->depth];
     vox_ctx* ctx = s.ctx;
     if (ctx->p.batch > 1 && !h_tet_offsets) return VOX_EINVAL;
@@ -1922,13 +1978,17 @@ static int pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const 
     char* a = s.base;
     // copy-in stream
     if (V > 0) PCK(cudaMemcpyAsync(a + A.verts, h_verts, (size_t)V * 12, cudaMemcpyHostToDevice, pipe->s_in));
-    if (T > 0) PCK(cudaMemcpyAsync(a + A.tets, h_tets, (size_t)T * 16, cudaMemcpyHostToDevice, pipe->s_in));
+    if (lat.cx)  // the keep mask (one byte per cell) travels in the slot's tet region
+        PCK(cudaMemcpyAsync(a + A.tets, lat.h_keep, (size_t)(T / 6), cudaMemcpyHostToDevice, pipe->s_in));
+    else if (T > 0) PCK(cudaMemcpyAsync(a + A.tets, h_tets, (size_t)T * 16, cudaMemcpyHostToDevice, pipe->s_in));
     if (ctx->p.batch > 1)
         PCK(cudaMemcpyAsync(a + A.off, h_tet_offsets, ((size_t)ctx->p.batch + 1) * 8, cudaMemcpyHostToDevice, pipe->s_in));
     PCK(cudaEventRecord(s.in_done, pipe->s_in));
     // compute stream
     PCK(cudaStreamWaitEvent(pipe->s_run, s.in_done, 0));
-    int rc = vox_tets(ctx, (const int32_t*)(a + A.verts), V, (const int32_t*)(a + A.tets), T, (const int64_t*)(a + A.off));
+    int rc = lat.cx ? vox_lattice(ctx, (const int32_t*)(a + A.verts), lat.cx, lat.cy, lat.cz, (const uint8_t*)(a + A.tets))
+                    : vox_tets(ctx, (const int32_t*)(a + A.verts), V, (const int32_t*)(a + A.tets), T,
+                               (const int64_t*)(a + A.off));
     if (rc) return rc;
     size_t out_bytes = vox_grid_words(ctx) * 4;
     if (cap_tiles < 0) {

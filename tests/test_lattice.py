@@ -1,0 +1,87 @@
+"""Lattice input (include/vox.h "vox_lattice"): the same mesh given as lattice vertices + a keep
+mask instead of a tet array must voxelize to the same bits as the oracle computes on the tets written out."""
+import numpy as np
+import pytest
+
+import meshgen
+import oracle
+from meshgen.kuhn import Mesh, kuhn_mesh, _uniform_corners
+
+
+def test_lattice_form_round_trips():
+    m = meshgen.make_config("cfg2")
+    keep = meshgen.lattice_form(m, (32, 32, 32))
+    assert keep.dtype == np.uint8 and keep.shape == (32 ** 3,)
+    assert int(np.unpackbits(keep).sum()) == m.T
+    c = _uniform_corners(32)
+    _v, t_all = kuhn_mesh(c, c, c, 0.0, None)           # connectivity only
+    present = ((keep[:, None] >> np.arange(6)) & 1).astype(bool).reshape(-1)
+    assert np.array_equal(t_all[present], m.tets)
+    full = meshgen.make_config("cfg1")
+    assert np.all(meshgen.lattice_form(full, (4, 4, 4)) == 63)
+
+
+def _cases():
+    rng = np.random.default_rng(44)
+    out = []
+    m = meshgen.carve_sphere(meshgen.make_config("cfg1"))
+    out.append(("cfg1_sphere", m, (4, 4, 4)))
+    out.append(("cfg2", meshgen.make_config("cfg2"), (32, 32, 32)))
+    out.append(("cfg4_small_drop3", meshgen.carve_every_third(meshgen.make_config("cfg4_small")), (32, 32, 32)))
+    # anisotropic lattice (different cell counts per axis), random carve, ragged grid
+    xs, ys, zs = (np.rint(np.linspace(0, e, n + 1)).astype(np.int64) for e, n in ((96 * 8, 5), (40 * 8, 3), (24 * 8, 7)))
+    v, t = kuhn_mesh(xs, ys, zs, 0.2, rng)
+    t = t[rng.random(len(t)) < 0.6]
+    out.append(("aniso", Mesh("aniso", v, t, (96, 40, 24), (96 * 8, 40 * 8, 24 * 8)), (5, 3, 7)))
+    return out
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("idx", range(4))
+def test_gpu_lattice_input_matches_oracle(idx):
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    name, m, cells = _cases()[idx]
+    exp = oracle.voxelize(m.verts, m.tets, m.grid, m.extent)
+    keep = meshgen.lattice_form(m, cells)
+    vz = pkg.Voxelizer(m.grid, m.extent)
+    vz.set_lattice(torch.from_numpy(m.verts).cuda(), cells, torch.from_numpy(keep).cuda())
+    pairs = vz.plan()
+    got = vz.run().cpu().numpy().view(np.uint32)
+    st = vz.status()
+    vz.close()
+    assert np.array_equal(got, exp), f"{name}: {(got != exp).sum()} words differ"
+    # the same pairs as with the tets written out
+    ref = pkg.voxelize(m.verts, m.tets, m.grid, m.extent)
+    assert np.array_equal(ref, exp) and pkg.voxelize.last_status["pairs"] == st["pairs"] == pairs
+
+
+@pytest.mark.gpu
+def test_gpu_lattice_through_the_pipe_dense_and_sparse():
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+    from oracle import sparse
+
+    name, m, cells = _cases()[1]
+    exp = oracle.voxelize(m.verts, m.tets, m.grid, m.extent)
+    keep = meshgen.lattice_form(m, cells)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    pipe = pkg.Pipe(m.grid, m.extent, depth=3, max_V=m.V, max_T=6 * cells[0] * cells[1] * cells[2])
+    ts = pipe.tile_shape
+    nb = ts["nbx"] * ts["nby"] * ts["nbz"]
+    nx, ny, nz = m.grid
+    h_out = torch.empty((1, nz, ny, nx // 32), dtype=torch.int32).pin_memory()
+    h_tab = torch.zeros(nb, dtype=torch.int32).pin_memory()
+    h_pay = torch.zeros((nb, ts["tz"], ts["ty"]), dtype=torch.int32).pin_memory()
+    t0 = pipe.submit_lattice(pin(m.verts), cells, pin(keep), h_out)
+    t1 = pipe.submit_lattice(pin(m.verts), cells, pin(keep), h_tab, h_pay, nb)
+    t2 = pipe.submit(pin(m.verts), pin(m.tets), h_out.clone().pin_memory())     # explicit tets after a lattice job
+    pipe.wait(t0)
+    st = pipe.wait(t1)
+    pipe.wait(t2)
+    pipe.close()
+    assert np.array_equal(h_out.numpy().view(np.uint32), exp)
+    assert sparse.check_table(h_tab.numpy(), h_pay.numpy(), exp, ts["ty"], ts["tz"]) == st["mixed_tiles"]
