@@ -394,6 +394,52 @@ def run_b200(args):
                           "mixed_tiles": sp_stats["mixed_tiles"], "full_tiles": sp_stats["full_tiles"], "tiles": nb,
                           "api": f"vox_pipe_submit_sparse/vox_pipe_wait, depth {depth}; payload stored by K4 "
                                  "into pinned host memory"}
+            # lattice input through the same pipeline (vox_pipe_submit_lattice): the mesh travels as lattice
+            # vertices + one keep byte per cell, no tet array (f4); sparse output as above
+            e2e_lattice = None
+            if getattr(m, "cells", None) is not None and m.batch == 1:
+                import meshgen as _mg
+
+                cells = m.cells
+                hk = torch.from_numpy(_mg.lattice_form(m, cells)).pin_memory()
+                lat_T = 6 * cells[0] * cells[1] * cells[2]
+                lpipe = pkg.Pipe(m.grid, m.extent, 1, depth=depth, max_V=m.V, max_T=lat_T, tile=args.tile,
+                                 variant=args.variant, max_pairs=pairs)
+                lts = lpipe.tile_shape
+                lnb = lts["nbx"] * lts["nby"] * lts["nbz"]
+                ltabs = [torch.zeros(lnb, dtype=torch.int32).pin_memory() for _ in range(depth)]
+                lpays = [torch.zeros((max(cap_tiles, 1), lts["tz"], lts["ty"]), dtype=torch.int32).pin_memory()
+                         for _ in range(depth)]
+
+                def lat_steps(k, sparse_out):
+                    tickets, last = [], None
+                    for i in range(k):
+                        if i >= depth:
+                            lpipe.wait(tickets[i - depth])
+                        if sparse_out:
+                            tickets.append(lpipe.submit_lattice(hv, cells, hk, ltabs[i % depth], lpays[i % depth], cap_tiles))
+                        else:
+                            tickets.append(lpipe.submit_lattice(hv, cells, hk, houts[i % depth]))
+                    for t in tickets[max(0, k - depth):]:
+                        last = lpipe.wait(t)
+                    return last
+
+                res = {}
+                for key, sp in (("dense", False), ("sparse", True)):
+                    lat_steps(max(3, depth), sp)
+                    torch.cuda.synchronize()
+                    t0 = time.perf_counter()
+                    lst = lat_steps(args.e2e_steps, sp)
+                    torch.cuda.synchronize()
+                    lms = (time.perf_counter() - t0) * 1e3
+                    res[key] = {"value": ssum * args.e2e_steps / (lms * 1e-3) / 1e9, "ms_per_step": lms / args.e2e_steps}
+                same_l = bool(torch.equal(houts[0], out.cpu()))
+                e2e_lattice = {"unit": UNIT, "h2d_bytes_per_step": hv.numel() * 4 + hk.numel(), "cells": list(cells),
+                               "dense_output": res["dense"], "sparse_output": res["sparse"], "same_result": same_l,
+                               "pairs": lst["pairs"],
+                               "api": f"vox_pipe_submit_lattice/vox_pipe_wait, depth {depth}"}
+                lpipe.close()
+                del ltabs, lpays
             pipe.close()
             del htabs, hpays
             # unpipelined single call
@@ -417,7 +463,7 @@ def run_b200(args):
                    "same_result": same,
                    "unpipelined_vox_run_host": {"ms_per_call": sync_ms,
                                                 "value": float(samples) / (sync_ms * 1e-3) / 1e9},
-                   "sparse_output": e2e_sparse}
+                   "sparse_output": e2e_sparse, "lattice_input": e2e_lattice}
             e2e_sparse["h2d_bytes_per_step"] = h2d
 
         if rank != 0:

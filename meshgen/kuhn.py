@@ -38,6 +38,7 @@ class Mesh:
     extent: tuple = (E_LATTICE, E_LATTICE, E_LATTICE)
     tet_offsets: np.ndarray = field(default=None)  # int64 [batch+1]
     expect_all_ones: bool = False  # union of the tets is the closed box [0,E]^3
+    cells: tuple = None  # (cx, cy, cz) when verts/tets come from kuhn_mesh of that lattice (see lattice_form)
 
     def __post_init__(self):
         if self.tet_offsets is None:
@@ -147,7 +148,7 @@ def _cfg1(seed):
     rng = np.random.default_rng(seed)
     c = _uniform_corners(4)
     v, t = kuhn_mesh(c, c, c, 0.2, rng)
-    return Mesh("cfg1_tiny_kuhn4", v, t, (32, 32, 32), expect_all_ones=True)
+    return Mesh("cfg1_tiny_kuhn4", v, t, (32, 32, 32), expect_all_ones=True, cells=(4, 4, 4))
 
 
 def _cfg2(seed):
@@ -156,7 +157,7 @@ def _cfg2(seed):
     v, t = kuhn_mesh(c, c, c, 0.2, rng)
     E = E_LATTICE
     t = _keep(v, t, lambda p: _in_sphere(p, (E / 2, E / 2, E / 2), 0.45 * E))
-    return Mesh("cfg2_sphere_kuhn32", v, t, (128, 128, 128))
+    return Mesh("cfg2_sphere_kuhn32", v, t, (128, 128, 128), cells=(32, 32, 32))
 
 
 def _cfg3_one(seed):
@@ -237,7 +238,7 @@ def _cfg4(seed, cells=128, grid=1024):
     for s in range(0, len(t), step):
         parts.append(_keep(v, t[s : s + step], pred))
     t = np.concatenate(parts)
-    return Mesh(f"cfg4_thingi_kuhn{cells}", v, t, (grid, grid, grid))
+    return Mesh(f"cfg4_thingi_kuhn{cells}", v, t, (grid, grid, grid), cells=(cells, cells, cells))
 
 
 def _cfg5(seed):
@@ -254,21 +255,22 @@ def _cfg5(seed):
     zs = np.concatenate([[0], np.cumsum(wz)])
     assert xs[-1] == E and zs[-1] == E and np.all(np.diff(xs) > 0) and np.all(np.diff(zs) > 0)
     v, t = kuhn_mesh(xs, ys, zs, 0.1, rng)
-    return Mesh("cfg5_graded_stress", v, t, (512, 512, 512), expect_all_ones=True)
+    return Mesh("cfg5_graded_stress", v, t, (512, 512, 512), expect_all_ones=True,
+                cells=(len(xs) - 1, len(ys) - 1, len(zs) - 1))
 
 
 def _s1(seed, jitter=0.2):
     rng = np.random.default_rng(seed)
     c = _uniform_corners(2)
     v, t = kuhn_mesh(c, c, c, jitter, rng)
-    return Mesh("s1_giant_tets", v, t, (512, 512, 512), expect_all_ones=True)
+    return Mesh("s1_giant_tets", v, t, (512, 512, 512), expect_all_ones=True, cells=(2, 2, 2))
 
 
 def _s2(seed, cells):
     rng = np.random.default_rng(seed)
     c = _uniform_corners(cells)
     v, t = kuhn_mesh(c, c, c, 0.2, rng)
-    return Mesh(f"s2_table1_kuhn{cells}", v, t, (256, 256, 256), expect_all_ones=True)
+    return Mesh(f"s2_table1_kuhn{cells}", v, t, (256, 256, 256), expect_all_ones=True, cells=(cells, cells, cells))
 
 
 _CONFIGS = {
