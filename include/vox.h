@@ -153,7 +153,7 @@ int vox_occupancy(void* cuda_stream, const uint32_t* d_bits_fine, int nx, int ny
  * only the fixed part. */
 int vox_validate(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes);
 
-/* End-to-end convenience for HOST buffers (the call the e2e benchmark times):
+/* End-to-end convenience for HOST buffers, one mesh, fully serialised (vox_pipe_* below overlaps the copies):
  * copies h_verts / h_tets / h_tet_offsets into the caller's device arena, runs
  * vox_tets + vox_run on `cuda_stream`, copies the grid to h_bits_out and
  * synchronises.  Host buffers should be pinned.  Arena layout is private;
