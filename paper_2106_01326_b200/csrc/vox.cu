@@ -890,11 +890,7 @@ __device__ __forceinline__ int span_bound(int r, int mx, int inv) {
     return c0 + (v >> 31);
 }
 
-__device__ __forceinline__ void smem_or(u32 saddr, u32 v) {
-    asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
-}
-
-template <int NLO, bool UNCOND>
+template <int NLO>
 __device__ __forceinline__ void raster_span(const int* rec, int lane, int img_stride) {
     const int4 MX = *reinterpret_cast<const int4*>(rec);
     const int4 MY = *reinterpret_cast<const int4*>(rec + 4);
@@ -916,30 +912,24 @@ __device__ __forceinline__ void raster_span(const int* rec, int lane, int img_st
         else { lower = max(max(-1, b0), max(b1, b2)); upper = min(A.y, b3); }
         const int n = upper - lower;  // number of solid voxels in the row (<= 0: none)
         const u32 saddr = (u32)B.x + 4u * (u32)(zz * img_stride + yy);
-        if (UNCOND) {
-            // branch-free: PTX shifts clamp at 32, so n <= 0 gives word 0 and the OR is a no-op
-            asm volatile(
-                "{\n\t.reg .b32 m, s;\n\t"
-                "sub.s32 s, 32, %1;\n\t"
-                "shr.b32 m, 0xFFFFFFFF, s;\n\t"
-                "add.s32 s, %2, %3;\n\t"
-                "shl.b32 m, m, s;\n\t"
-                "red.shared.or.b32 [%0], m;\n\t}"
-                ::"r"(saddr), "r"(n), "r"(lower), "r"(A.x)
-                : "memory");
-        } else if (n > 0) {
-            smem_or(saddr, (0xFFFFFFFFu >> (32 - n)) << (lower + A.x));
-        }
+        // branch-free: PTX shifts clamp at 32, so n <= 0 gives word 0 and the OR is a no-op
+        asm volatile(
+            "{\n\t.reg .b32 m, s;\n\t"
+            "sub.s32 s, 32, %1;\n\t"
+            "shr.b32 m, 0xFFFFFFFF, s;\n\t"
+            "add.s32 s, %2, %3;\n\t"
+            "shl.b32 m, m, s;\n\t"
+            "red.shared.or.b32 [%0], m;\n\t}"
+            ::"r"(saddr), "r"(n), "r"(lower), "r"(A.x)
+            : "memory");
     }
 }
 
-// SPARSE: instead of the dense grid the CTA writes one table word for its tile (TILE_EMPTY, TILE_FULL or
-// 1 + payload slot) and, for a mixed tile only, its TY*TZ row words contiguously into payload[slot]
-// (which may be host-mapped pinned memory: the copy-out is then fused into the kernel's stores).
-template <int NT, int MINB, bool UNCOND, bool SPARSE>
+// (kept as vox_set_variant 3 for A/B runs and parity: warp per pair, lanes = rows; dense output only)
+template <int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restrict__ offsets,
                                                     const u32* __restrict__ list, u32* __restrict__ bits,
-                                                    u32* __restrict__ hdr, SparseOut so) {
+                                                    u32* __restrict__ hdr) {
     __shared__ u32 img[32 * (32 + IMG_SKEW)];
     __shared__ __align__(16) int rec[NT][SREC_W];
     __shared__ u32 s_large;
@@ -959,10 +949,6 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
     for (int i = tid; i < img_words; i += NT) img[i] = 0;
     if (tid == 0) s_large = 0;
     const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
-    if (SPARSE && beg >= end) {  // no tets: empty tile, nothing else to do
-        if (tid == 0) so.table[b] = TILE_EMPTY;
-        return;
-    }
     u32 seen_large = 0;
     for (u32 base = beg; base < end; base += NT) {
         __syncthreads();
@@ -977,9 +963,9 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
             const int info = r[R_INFO];
             // nlo == 0 or 4 cannot happen for a non-degenerate tet (the four sigma*N sum to zero
             // and planes with N_x == 0 count as hi-type); KIND_LARGE (info >= 256) is drawn below
-            if (info == 2) raster_span<2, UNCOND>(r, lane, img_stride);
-            else if (info == 1) raster_span<1, UNCOND>(r, lane, img_stride);
-            else if (info == 3) raster_span<3, UNCOND>(r, lane, img_stride);
+            if (info == 2) raster_span<2>(r, lane, img_stride);
+            else if (info == 1) raster_span<1>(r, lane, img_stride);
+            else if (info == 3) raster_span<3>(r, lane, img_stride);
         }
         // large pairs of this batch (rare): kept out of the loop above so that it holds no call
         const u32 nl = s_large;  // cumulative; stable between the barrier above and the next one
@@ -994,49 +980,11 @@ __global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restr
     __syncthreads();
     const int rows = 1 << (p.ty_log + p.tz_log);
     if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
-    if (!SPARSE) {
-        for (int i = tid; i < rows; i += NT) {
-            const int z = i >> p.ty_log, y = i & (TY - 1);
-            const int gy = Y0 + y, gz = Z0 + z;
-            if (gy < p.ny && gz < p.nz)
-                bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[z * img_stride + y];
-        }
-        return;
-    }
-    // classify over the rows that lie inside the grid (ragged last tiles)
-    __shared__ u32 s_slot;
-    u32 all = 0xFFFFFFFFu, any = 0u;
     for (int i = tid; i < rows; i += NT) {
         const int z = i >> p.ty_log, y = i & (TY - 1);
-        if (Y0 + y < p.ny && Z0 + z < p.nz) {
-            const u32 w = img[z * img_stride + y];
-            all &= w;
-            any |= w;
-        }
-    }
-    const int is_full = __syncthreads_and(all == 0xFFFFFFFFu);
-    const int is_any = __syncthreads_or(any != 0u);
-    if (!is_any || is_full) {
-        if (tid == 0) {
-            so.table[b] = is_full ? TILE_FULL : TILE_EMPTY;
-            if (is_full) atomicAdd(hdr + H_FULL, 1u);
-        }
-        return;
-    }
-    if (tid == 0) {
-        const u32 slot = atomicAdd(hdr + H_MIXED, 1u);
-        s_slot = slot;
-        so.table[b] = slot < so.cap ? slot + 1u : TILE_DROPPED;
-        if (slot >= so.cap) hdr[H_PAYLOAD_OVERFLOW] = 1;
-    }
-    __syncthreads();
-    const u32 slot = s_slot;
-    if (slot >= so.cap) return;
-    u32* dst = so.payload + (size_t)slot * rows;
-    for (int i = tid; i < rows; i += NT) {
-        const int z = i >> p.ty_log, y = i & (TY - 1);
-        const bool in = (Y0 + y < p.ny) && (Z0 + z < p.nz);
-        dst[i] = in ? img[z * img_stride + y] : 0u;
+        const int gy = Y0 + y, gz = Z0 + z;
+        if (gy < p.ny && gz < p.nz)
+            bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[z * img_stride + y];
     }
 }
 
@@ -1593,15 +1541,9 @@ static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t w
     const SparseOut so = ctx->sparse;
     if (so.table) {
         k4_flat<128, 8, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);
-    } else switch (ctx->variant) {  // A/B variants kept for the parity tests and the sweep in DESIGN.md
+    } else switch (ctx->variant) {  // A/B variants kept for the parity tests and the history in DESIGN.md
         case 1: k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
-        case 2: k4_span<256, 4, true, false><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
-        case 4: k4_span<128, 8, false, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
-        case 5: k4_span<128, 7, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
-        case 6: k4_span<128, 9, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
-        case 3: k4_span<128, 8, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
-        case 7: k4_flat<128, 7, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
-        case 8: k4_flat<256, 4, false><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr, so); break;
+        case 3: k4_span<128, 8><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
         default: k4_flat<128, 8, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);  // 64 regs, 32 warps/SM
     }
     CK(cudaGetLastError());
