@@ -273,6 +273,11 @@ def run_b200(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    if not os.path.exists(pkg.lib_path()):  # a fresh checkout: compile the extension (no-op otherwise)
+        from paper_2106_01326_b200.build import build as _build
+
+        if local_rank == 0:
+            _build()
     pkg.load_library()  # fail loudly if libvox.so is missing
     torch.cuda.set_device(local_rank)
     dist = None
