@@ -278,6 +278,11 @@ def run_b200(args):
 
         if local_rank == 0:
             _build()
+        else:  # the other ranks of the node wait for rank 0's build
+            for _ in range(600):
+                if os.path.exists(pkg.lib_path()):
+                    break
+                time.sleep(0.5)
     pkg.load_library()  # fail loudly if libvox.so is missing
     torch.cuda.set_device(local_rank)
     dist = None
