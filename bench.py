@@ -407,18 +407,27 @@ def run_b200(args):
             # lattice input through the same pipeline (vox_pipe_submit_lattice): the mesh travels as lattice
             # vertices + one keep byte per cell, no tet array (f4); sparse output as above
             e2e_lattice = None
-            if getattr(m, "cells", None) is not None and m.batch == 1:
+            if getattr(m, "cells", None) is not None:
                 import meshgen as _mg
 
                 cells = m.cells
                 hk = torch.from_numpy(_mg.lattice_form(m, cells)).pin_memory()
-                lat_T = 6 * cells[0] * cells[1] * cells[2]
-                lpipe = pkg.Pipe(m.grid, m.extent, 1, depth=depth, max_V=m.V, max_T=lat_T, tile=args.tile,
-                                 variant=args.variant, max_pairs=pairs)
+                lat_T = m.batch * 6 * cells[0] * cells[1] * cells[2]
+                # the implicit tet count picks its own tile: plan once for the exact pair count (outside the timing)
+                vzl = pkg.Voxelizer(m.grid, m.extent, m.batch, tile=args.tile, variant=args.variant)
+                d_keep = hk.cuda()
+                vzl.set_lattice(d_verts, cells, d_keep)
+                lat_pairs = vzl.plan(stream)
+                vzl.run(stream=stream)
+                lat_cap = max(int(vzl.status(stream)["nonempty_tiles"]), 1)  # its tiles differ from the tet-array run's
+                vzl.close()
+                del d_keep
+                lpipe = pkg.Pipe(m.grid, m.extent, m.batch, depth=depth, max_V=m.V, max_T=lat_T, tile=args.tile,
+                                 variant=args.variant, max_pairs=lat_pairs)
                 lts = lpipe.tile_shape
-                lnb = lts["nbx"] * lts["nby"] * lts["nbz"]
+                lnb = m.batch * lts["nbx"] * lts["nby"] * lts["nbz"]
                 ltabs = [torch.zeros(lnb, dtype=torch.int32).pin_memory() for _ in range(depth)]
-                lpays = [torch.zeros((max(cap_tiles, 1), lts["tz"], lts["ty"]), dtype=torch.int32).pin_memory()
+                lpays = [torch.zeros((lat_cap, lts["tz"], lts["ty"]), dtype=torch.int32).pin_memory()
                          for _ in range(depth)]
 
                 def lat_steps(k, sparse_out):
@@ -427,7 +436,7 @@ def run_b200(args):
                         if i >= depth:
                             lpipe.wait(tickets[i - depth])
                         if sparse_out:
-                            tickets.append(lpipe.submit_lattice(hv, cells, hk, ltabs[i % depth], lpays[i % depth], cap_tiles))
+                            tickets.append(lpipe.submit_lattice(hv, cells, hk, ltabs[i % depth], lpays[i % depth], lat_cap))
                         else:
                             tickets.append(lpipe.submit_lattice(hv, cells, hk, houts[i % depth]))
                     for t in tickets[max(0, k - depth):]:

@@ -85,7 +85,8 @@ int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const int32_t* d_t
  * (i*(cy+1) + j)*(cz+1) + k; cell (i,j,k), index c = (i*cy + j)*cz + k, is split into the 6 Kuhn tets, tet q
  * walking from the cell's low corner along the axes of the q-th permutation of (x,y,z) in lexicographic order
  * (xyz, xzy, yxz, yzx, zxy, zyx); bit q of d_keep[c] says whether tet q is present.  Equivalent to vox_tets with
- * the 6*cx*cy*cz tets written out (absent ones dropped); batch must be 1.  vox_status counts only present tets
+ * the 6*cx*cy*cz tets written out (absent ones dropped).  With batch > 1 every mesh has the same lattice dims:
+ * mesh m's vertices and keep bytes are the m-th block of d_verts / d_keep.  vox_status counts only present tets
  * as culled. */
 int vox_lattice(vox_ctx* ctx, const int32_t* d_verts, int cx, int cy, int cz, const uint8_t* d_keep);
 
@@ -217,7 +218,8 @@ int vox_pipe_submit_sparse(vox_pipe* pipe, const int32_t* h_verts, int64_t V, co
                            int64_t payload_capacity_tiles, int64_t* ticket_out);
 /* Lattice input through the pipe (vox_lattice): h_verts int32[(cx+1)(cy+1)(cz+1)][3] and h_keep uint8[cx*cy*cz],
  * pinned.  payload_capacity_tiles < 0: dense (h_out = the grid); otherwise sparse (h_out = tile table, h_payload as
- * in vox_pipe_submit_sparse).  The pipe must have been created with max_T >= 6*cx*cy*cz. */
+ * in vox_pipe_submit_sparse).  The pipe must have been created with max_T >= batch*6*cx*cy*cz and
+ * max_V >= batch*(cx+1)(cy+1)(cz+1). */
 int vox_pipe_submit_lattice(vox_pipe* pipe, const int32_t* h_verts, int cx, int cy, int cz, const uint8_t* h_keep,
                             uint32_t* h_out, uint32_t* h_payload, int64_t payload_capacity_tiles, int64_t* ticket_out);
 int vox_pipe_wait(vox_pipe* pipe, int64_t ticket, int64_t stats_out[6]);

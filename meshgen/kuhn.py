@@ -200,6 +200,7 @@ def _cfg3(seed, n_meshes=256):
         np.concatenate(ts).astype(np.int32),
         (64, 64, 64),
         tet_offsets=np.array(offs, dtype=np.int64),
+        cells=(24, 24, 24),
     )
 
 
@@ -319,9 +320,16 @@ def lattice_form(m: Mesh, cells) -> np.ndarray:
     the cell's q-th tet (q = index into the lexicographic permutations of the axes, as kuhn_mesh lists them) is in
     m.tets.  With m.verts this is the lattice input of include/vox.h ("vox_lattice"); m.tets is the same mesh
     written out.  Pure index bookkeeping."""
-    assert m.batch == 1
     cx, cy, cz = (int(c) for c in cells)
-    assert m.V == (cx + 1) * (cy + 1) * (cz + 1)
+    vm = (cx + 1) * (cy + 1) * (cz + 1)
+    assert m.V == m.batch * vm
+    if m.batch > 1:  # a batch of meshes on the same lattice dims: one block of keep bytes per mesh
+        parts = []
+        for b in range(m.batch):
+            lo, hi = int(m.tet_offsets[b]), int(m.tet_offsets[b + 1])
+            one = Mesh(m.name, m.verts[b * vm:(b + 1) * vm], m.tets[lo:hi] - b * vm, m.grid, m.extent)
+            parts.append(lattice_form(one, cells))
+        return np.concatenate(parts)
     t = m.tets.astype(np.int64)
     v0 = t[:, 0]
     k = v0 % (cz + 1)

@@ -187,11 +187,12 @@ class Voxelizer:
         cx, cy, cz = (int(c) for c in cells)
         assert verts.is_cuda and verts.dtype == torch.int32 and verts.is_contiguous()
         assert keep.is_cuda and keep.dtype == torch.uint8 and keep.is_contiguous()
-        assert verts.numel() == 3 * (cx + 1) * (cy + 1) * (cz + 1) and keep.numel() == cx * cy * cz
+        assert verts.numel() == self.batch * 3 * (cx + 1) * (cy + 1) * (cz + 1)
+        assert keep.numel() == self.batch * cx * cy * cz
         self._ck(self._lib.vox_lattice(self._ctx, ctypes.c_void_p(verts.data_ptr()), cx, cy, cz,
                                        ctypes.c_void_p(keep.data_ptr())), "vox_lattice")
         self._keep = (verts, keep)
-        self.T, self.V = 6 * cx * cy * cz, (cx + 1) * (cy + 1) * (cz + 1)
+        self.T, self.V = self.batch * 6 * cx * cy * cz, self.batch * (cx + 1) * (cy + 1) * (cz + 1)
 
     def alloc_workspace(self, nbytes=None):
         torch = _torch_cuda()
@@ -268,7 +269,8 @@ class Voxelizer:
         return self._last_sparse
 
     def status(self, stream=None):
-        """Synchronises.  Returns dict(pairs, culled, large_pairs, nonempty_tiles); raises on overflow."""
+        """Synchronises.  Returns dict(pairs, culled, large_pairs, nonempty_tiles) of the last run() on this
+        workspace; raises on overflow.  (plan() may re-allocate the workspace: call status() after run().)"""
         torch = _torch_cuda()
         st = (ctypes.c_int64 * 4)()
         rc = self._lib.vox_status(self._ctx, _stream_ptr(torch, stream), ctypes.c_void_p(self._ws.data_ptr()), st)
@@ -401,7 +403,8 @@ class Pipe:
             assert not t.is_cuda and t.is_contiguous() and (t.numel() == 0 or t.is_pinned()), \
                 "pipe buffers must be pinned CPU tensors"
         cx, cy, cz = (int(c) for c in cells)
-        assert h_verts.numel() == 3 * (cx + 1) * (cy + 1) * (cz + 1) and h_keep.numel() == cx * cy * cz
+        assert h_verts.numel() == self.batch * 3 * (cx + 1) * (cy + 1) * (cz + 1)
+        assert h_keep.numel() == self.batch * cx * cy * cz
         ticket = ctypes.c_int64(-1)
         self._ck(
             self._lib.vox_pipe_submit_lattice(self._p, ctypes.c_void_p(h_verts.data_ptr()), cx, cy, cz,

@@ -130,12 +130,15 @@ struct Tet {
 __device__ __forceinline__ int4 lattice_ids(const Params& p, i64 t) {
     const int q = (int)(t % 6);
     i64 c = t / 6;
+    const i64 cells = (i64)p.lcx * p.lcy * p.lcz;
+    const int mesh = (int)(c / cells);  // batch: mesh m owns cells [m*cells, (m+1)*cells) and its own vertex block
+    c -= mesh * cells;
     const int k = (int)(c % p.lcz);
     c /= p.lcz;
     const int j = (int)(c % p.lcy);
     const int i = (int)(c / p.lcy);
     const int sz = 1, sy = p.lcz + 1, sx = (p.lcy + 1) * (p.lcz + 1);
-    const int v0 = (i * (p.lcy + 1) + j) * (p.lcz + 1) + k;
+    const int v0 = mesh * (p.lcx + 1) * sx + (i * (p.lcy + 1) + j) * (p.lcz + 1) + k;
     // permutations of (x,y,z), lexicographic: xyz xzy yxz yzx zxy zyx
     const int a1 = (q < 2) ? sx : (q < 4) ? sy : sz;
     const int a3 = (q == 3 || q == 5) ? sx : (q == 1 || q == 4) ? sy : sz;
@@ -174,6 +177,7 @@ __device__ __forceinline__ void axis_range(int a, int b, int c, int d, int h, in
 
 __device__ __forceinline__ int mesh_of(const Params& p, i64 t) {
     if (p.batch == 1) return 0;
+    if (p.lcx) return (int)(t / (6ll * p.lcx * p.lcy * p.lcz));  // lattice input: equal blocks per mesh
     int lo = 0, hi = p.batch;  // off[lo] <= t < off[hi]
     while (hi - lo > 1) {
         int mid = (lo + hi) >> 1;
@@ -1401,8 +1405,7 @@ extern "C" int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const i
 
 extern "C" int vox_lattice(vox_ctx* ctx, const int32_t* d_verts, int cx, int cy, int cz, const uint8_t* d_keep) {
     if (!ctx || cx < 1 || cy < 1 || cz < 1 || !d_verts || !d_keep) return VOX_EINVAL;
-    if (ctx->p.batch != 1) return VOX_EINVAL;
-    const i64 cells = (i64)cx * cy * cz, V = (i64)(cx + 1) * (cy + 1) * (cz + 1);
+    const i64 cells = (i64)ctx->p.batch * cx * cy * cz, V = (i64)ctx->p.batch * (cx + 1) * (cy + 1) * (cz + 1);
     if (6 * cells > 0xFFFFFFF0ll || V > 0x7FFFFFFFll) return VOX_ERANGE;
     Params& p = ctx->p;
     p.verts = d_verts;
@@ -1895,8 +1898,10 @@ extern "C" int vox_pipe_submit_lattice(vox_pipe* pipe, const int32_t* h_verts, i
                                        int64_t payload_capacity_tiles, int64_t* ticket_out) {
     if (cx < 1 || cy < 1 || cz < 1 || !h_keep || !h_verts) return VOX_EINVAL;
     if (payload_capacity_tiles > 0 && !h_payload) return VOX_EINVAL;
-    const int64_t cells = (int64_t)cx * cy * cz;
-    return pipe_submit(pipe, h_verts, (int64_t)(cx + 1) * (cy + 1) * (cz + 1), NULL, 6 * cells, NULL,
+    if (!pipe) return VOX_EINVAL;
+    const int64_t batch = pipe->slot[0].ctx->p.batch;
+    const int64_t cells = batch * cx * cy * cz;
+    return pipe_submit(pipe, h_verts, batch * (cx + 1) * (cy + 1) * (cz + 1), NULL, 6 * cells, NULL,
                        LatticeIn{cx, cy, cz, h_keep}, h_out, h_payload, payload_capacity_tiles < 0 ? -1 : payload_capacity_tiles,
                        ticket_out);
 }
@@ -1911,7 +1916,7 @@ static int pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const 
     if (T > 0 && (!h_verts || (!h_tets && !lat.cx))) return VOX_EINVAL;
     PipeSlot& s = pipe->slot[pipe->next_ticket % pipe->depth];
     vox_ctx* ctx = s.ctx;
-    if (ctx->p.batch > 1 && !h_tet_offsets) return VOX_EINVAL;
+    if (ctx->p.batch > 1 && !h_tet_offsets && !lat.cx) return VOX_EINVAL;
     if (s.ticket >= 0) {  // slot still in flight and never waited on: its result is complete but unclaimed
         PCK(cudaEventSynchronize(s.out_done));
         s.ticket = -1;
@@ -1923,7 +1928,7 @@ static int pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const 
     if (lat.cx)  // the keep mask (one byte per cell) travels in the slot's tet region
         PCK(cudaMemcpyAsync(a + A.tets, lat.h_keep, (size_t)(T / 6), cudaMemcpyHostToDevice, pipe->s_in));
     else if (T > 0) PCK(cudaMemcpyAsync(a + A.tets, h_tets, (size_t)T * 16, cudaMemcpyHostToDevice, pipe->s_in));
-    if (ctx->p.batch > 1)
+    if (ctx->p.batch > 1 && !lat.cx)
         PCK(cudaMemcpyAsync(a + A.off, h_tet_offsets, ((size_t)ctx->p.batch + 1) * 8, cudaMemcpyHostToDevice, pipe->s_in));
     PCK(cudaEventRecord(s.in_done, pipe->s_in));
     // compute stream

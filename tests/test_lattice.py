@@ -33,20 +33,22 @@ def _cases():
     v, t = kuhn_mesh(xs, ys, zs, 0.2, rng)
     t = t[rng.random(len(t)) < 0.6]
     out.append(("aniso", Mesh("aniso", v, t, (96, 40, 24), (96 * 8, 40 * 8, 24 * 8)), (5, 3, 7)))
+    b = meshgen.make_config("cfg3_small")                    # a batch of 4 meshes on the same 24^3 lattice
+    out.append(("cfg3_small", b, b.cells))
     return out
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("idx", range(4))
+@pytest.mark.parametrize("idx", range(5))
 def test_gpu_lattice_input_matches_oracle(idx):
     import torch
 
     import paper_2106_01326_b200 as pkg
 
     name, m, cells = _cases()[idx]
-    exp = oracle.voxelize(m.verts, m.tets, m.grid, m.extent)
+    exp = oracle.voxelize(m.verts, m.tets, m.grid, m.extent, tet_offsets=m.tet_offsets)
     keep = meshgen.lattice_form(m, cells)
-    vz = pkg.Voxelizer(m.grid, m.extent)
+    vz = pkg.Voxelizer(m.grid, m.extent, m.batch)
     vz.set_lattice(torch.from_numpy(m.verts).cuda(), cells, torch.from_numpy(keep).cuda())
     pairs = vz.plan()
     got = vz.run().cpu().numpy().view(np.uint32)
@@ -54,7 +56,7 @@ def test_gpu_lattice_input_matches_oracle(idx):
     vz.close()
     assert np.array_equal(got, exp), f"{name}: {(got != exp).sum()} words differ"
     # the same pairs as with the tets written out
-    ref = pkg.voxelize(m.verts, m.tets, m.grid, m.extent)
+    ref = pkg.voxelize(m.verts, m.tets, m.grid, m.extent, tet_offsets=m.tet_offsets if m.batch > 1 else None)
     assert np.array_equal(ref, exp) and pkg.voxelize.last_status["pairs"] == st["pairs"] == pairs
 
 
@@ -85,3 +87,24 @@ def test_gpu_lattice_through_the_pipe_dense_and_sparse():
     pipe.close()
     assert np.array_equal(h_out.numpy().view(np.uint32), exp)
     assert sparse.check_table(h_tab.numpy(), h_pay.numpy(), exp, ts["ty"], ts["tz"]) == st["mixed_tiles"]
+
+
+@pytest.mark.gpu
+def test_gpu_batched_lattice_through_the_pipe():
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    m = meshgen.make_config("cfg3_small")
+    exp = oracle.voxelize(m.verts, m.tets, m.grid, m.extent, tet_offsets=m.tet_offsets)
+    keep = meshgen.lattice_form(m, m.cells)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    pipe = pkg.Pipe(m.grid, m.extent, m.batch, depth=2, max_V=m.V, max_T=m.batch * 6 * 24 ** 3)
+    nx, ny, nz = m.grid
+    outs = [torch.empty((m.batch, nz, ny, nx // 32), dtype=torch.int32).pin_memory() for _ in range(2)]
+    ts = [pipe.submit_lattice(pin(m.verts), m.cells, pin(keep), o) for o in outs]
+    for t in ts:
+        pipe.wait(t)
+    pipe.close()
+    for o in outs:
+        assert np.array_equal(o.numpy().view(np.uint32), exp)
