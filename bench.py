@@ -564,7 +564,9 @@ def run_b200(args):
             "mtets_per_s": tsum * args.steps / sec / 1e6,
             "gvoxels_per_s": world * m.batch * nx * ny * nz * args.steps / sec / 1e9,
             "kernel_ms": shares, "status": st, "popcount": popcount,
-            "gpu_launches": 4 * (args.steps + ((2 * (args.e2e_steps + max(3, args.e2e_depth)) + 5) if e2e else 0)),
+            "gpu_launches": 4 * (args.steps + ((2 * (args.e2e_steps + max(3, args.e2e_depth)) + 5) if e2e else 0)
+                                 + ((2 * (args.e2e_steps + max(3, args.e2e_depth)) + 2)
+                                    if e2e and e2e.get("lattice_input") else 0)) + (23 if occ else 0),
             "clocks": clk.summary(), "roofline": roofline, "occupancy_fold": occ, "cpu_baseline": cpu, "e2e": e2e,
         }
         line["config"].pop("tile")
