@@ -27,7 +27,8 @@
  * allocates only the host-side context.  vox_run only enqueues work on the
  * given stream: no allocation, no host synchronisation.
  *
- * Pointers named d_* are DEVICE pointers, h_* are HOST pointers.
+ * Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  d_workspace must be
+ * 16-byte aligned (VOX_EINVAL otherwise), d_tets 16-byte aligned, d_bits_out 4-byte aligned.
  * `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
  *
  * Errors: every int-returning call returns VOX_OK (0) or a negative code;
@@ -48,7 +49,8 @@ typedef struct vox_ctx vox_ctx; /* opaque, host side */
 enum {
     VOX_OK = 0,
     VOX_EINVAL = -1,     /* null pointer, n <= 0, nx % 32 != 0, extent % (2n) != 0, batch < 1, V/T < 0 */
-    VOX_ERANGE = -2,     /* extent > 2^20 (the int64 bound 6*extent^3 < 2^63 would not hold), n > 32768 */
+    VOX_ERANGE = -2,     /* extent > 2^20 (the int64 bound 6*extent^3 < 2^63 would not hold), n > 32768,
+                            more than 2^31-1 tiles */
     VOX_EWORKSPACE = -3, /* workspace too small (at enqueue, or reported by vox_status after a run) */
     VOX_ECUDA = -4,      /* CUDA runtime error; text via vox_last_error */
     VOX_ESTATE = -5,     /* call order: vox_run before vox_tets, ... */
@@ -67,8 +69,8 @@ void vox_destroy(vox_ctx* ctx);
  * result of vox_run does not depend on the tile; vox_tile_shape reports it. */
 int vox_set_tile(vox_ctx* ctx, int ty, int tz);
 
-/* Optional: kernel variant of the brick voxelizer, 0 = default.  Result-neutral
- * (used by tests and the benchmark to compare variants). */
+/* Kernel variant of the brick voxelizer for A/B runs, 0 = default.  Result-neutral by contract.  No alternative
+ * is compiled in at present: any non-zero value is refused with VOX_EINVAL (never silently ignored). */
 int vox_set_variant(vox_ctx* ctx, int variant);
 
 /* Borrow the mesh.  d_verts int32[V][3] with coordinates in [0, extent];
@@ -242,6 +244,10 @@ int vox_timing_read(vox_ctx* ctx, int run, float ms_out[5]);
  * (fma pipe), 2 = mixed.  *ops_out = thread-level INT32 ops it executes. */
 int vox_probe_int32(void* cuda_stream, int kind, int blocks, int iters, uint32_t* d_sink,
                     double* ops_out);
+
+/* Number of CUDA kernels this library has launched in this process so far (all contexts and pipes; memsets and
+ * copies are not kernels).  bench.py reports the difference across its timed region as `gpu_launches`. */
+uint64_t vox_kernel_launches(void);
 
 const char* vox_strerror(int code);
 const char* vox_last_error(const vox_ctx* ctx); /* CUDA error text of the last VOX_ECUDA */

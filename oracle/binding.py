@@ -25,7 +25,7 @@ def build(force: bool = False) -> str:
         if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
             tmp = _LIB + f".tmp{os.getpid()}"
             subprocess.check_call(
-                ["gcc", "-O2", "-fopenmp", "-fwrapv", "-shared", "-fPIC", "-o", tmp, _SRC]
+                ["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC]
             )
             os.replace(tmp, _LIB)
     return _LIB

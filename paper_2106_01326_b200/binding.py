@@ -17,7 +17,7 @@ EXPORTS = [
     "vox_pipe_create", "vox_pipe_destroy", "vox_pipe_set_variant", "vox_pipe_set_tile", "vox_pipe_arena_bytes",
     "vox_pipe_bind", "vox_pipe_submit", "vox_pipe_wait", "vox_pipe_last_error",
     "vox_tile_shape", "vox_run_sparse", "vox_sparse_status", "vox_pipe_submit_sparse", "vox_pipe_tile_shape",
-    "vox_pipe_reserve_pairs", "vox_occupancy", "vox_lattice", "vox_pipe_submit_lattice",
+    "vox_pipe_reserve_pairs", "vox_occupancy", "vox_lattice", "vox_pipe_submit_lattice", "vox_kernel_launches",
 ]
 
 
@@ -81,6 +81,7 @@ def load_library():
         "vox_occupancy": (i32, [vp, vp, i32, i32, i32, i32, i32, vp]),
         "vox_lattice": (i32, [vp, vp, i32, i32, i32, vp]),
         "vox_pipe_submit_lattice": (i32, [vp, vp, i32, i32, i32, vp, vp, vp, i64, ctypes.POINTER(i64)]),
+        "vox_kernel_launches": (ctypes.c_uint64, []),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -501,6 +502,11 @@ def voxelize_host(verts, tets, grid, extent=(65536, 65536, 65536), tet_offsets=N
         return out.numpy().view(np.uint32)
     finally:
         vz.close()
+
+
+def kernel_launches() -> int:
+    """vox_kernel_launches: kernels launched by libvox.so in this process so far."""
+    return int(load_library().vox_kernel_launches())
 
 
 def probe_int32(kind=0, blocks=148 * 16, iters=4096, repeats=5):

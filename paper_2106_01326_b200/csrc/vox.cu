@@ -4,10 +4,10 @@
 //   K1 k1_count    per-tet voxel bbox -> tile range, sliver/degenerate cull, per-tile histogram
 //   K2 k2_scan     exclusive scan of the tile counts (+ cursors, totals)
 //   K3 k3_scatter  tet ids into per-tile lists
-//   K4 k4_brick    one CTA per 32 x TY x TZ tile: exact integer edge functions of
-//                  Theorem 1 stepped along rows, row words formed on
+//   K4 k4_flat     one CTA per 32 x TY x TZ tile: exact integer edge functions of
+//                  Theorem 1, one exact x-span per row, row words formed on
 //                  chip, tile image stored once (no global atomics on the grid)
-//   K5 (inside K4) large-tet path: exact tile classification + 64-bit ballot rasteriser
+//   K5 (inside K4) large-tet path: exact tile classification + int64 span rows / 64-bit ballot rasteriser
 //
 // Exactness: inside(P) <=> four affine functions G_k(P) >= 0, each an exact integer
 // (DESIGN.md "Arithmetic").  No floating point decides a bit.
@@ -81,6 +81,10 @@ enum { BIG_TILES = 64, BIG_CAP = 4096, RANGE_BIG = 0x40000000 };
 #define TILE_DROPPED 0xFFFFFFFEu
 
 static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// kernels launched by this library in this process (vox_kernel_launches: bench.py's gpu_launches)
+static unsigned long long g_launches = 0;
+static inline void count_launch() { __atomic_fetch_add(&g_launches, 1ull, __ATOMIC_RELAXED); }
 
 struct WsLayout {
     size_t hdr, counts, cursor, big, range, list, fixed_end;
@@ -479,181 +483,10 @@ __device__ __forceinline__ void tet_planes(const Params& p, const Tet& q, int X0
 __device__ __forceinline__ i64 iabs64(i64 v) { return v < 0 ? -v : v; }
 
 
-enum { REC_W = 18, KIND_FAST = 0, KIND_LARGE = 1 };
-// record: [0..3] mx, [4..7] my, [8..11] mz, [12..15] g0, [16] box, [17] kind | (for LARGE: [0] = tet id)
+enum { KIND_LARGE = 1 };
 
 __device__ __forceinline__ u32 pack_box(int x0, int x1, int y0, int y1, int z0, int z1) {
     return (u32)x0 | ((u32)x1 << 5) | ((u32)y0 << 10) | ((u32)y1 << 15) | ((u32)z0 << 20) | ((u32)z1 << 25);
-}
-
-// local (tile-relative) closed box of the tet's voxel bbox, intersected with the tile
-__device__ __forceinline__ u32 local_box(const Params& p, const Tet& q, int X0, int Y0, int Z0) {
-    int x0, x1, y0, y1, z0, z1;
-    axis_range(q.ax, q.bx, q.cx, q.dx, p.hx, p.qx, p.nx, x0, x1);
-    axis_range(q.ay, q.by, q.cy, q.dy, p.hy, p.qy, p.ny, y0, y1);
-    axis_range(q.az, q.bz, q.cz, q.dz, p.hz, p.qz, p.nz, z0, z1);
-    const int TY = 1 << p.ty_log, TZ = 1 << p.tz_log;
-    x0 = max(x0 - X0, 0); x1 = min(x1 - X0, 31);
-    y0 = max(y0 - Y0, 0); y1 = min(y1 - Y0, TY - 1);
-    z0 = max(z0 - Z0, 0); z1 = min(z1 - Z0, TZ - 1);
-    return pack_box(x0, x1, y0, y1, z0, z1);
-}
-
-// thread-per-tet setup: writes the record
-__device__ __forceinline__ void setup_record(const Params& p, u32 t, int X0, int Y0, int Z0, int* rec) {
-    Tet q = load_tet(p, t);
-    Planes P;
-    tet_planes(p, q, X0, Y0, Z0, P);
-    u32 box = local_box(p, q, X0, Y0, Z0);
-    bool fits = true;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        i64 bound = iabs64(P.g0[k]) + 31 * (iabs64(P.mx[k]) + iabs64(P.my[k]) + iabs64(P.mz[k]));
-        fits = fits && (bound < 0x7FFFFFFFll);
-    }
-    if (fits) {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            rec[k] = (int)P.mx[k];
-            rec[4 + k] = (int)P.my[k];
-            rec[8 + k] = (int)P.mz[k];
-            rec[12 + k] = (int)P.g0[k];
-        }
-        rec[17] = KIND_FAST;
-    } else {
-        rec[0] = (int)t;
-        rec[17] = KIND_LARGE;
-    }
-    rec[16] = (int)box;
-}
-
-// Fast path: all four G fit int32 over the whole tile.  Lanes = rows (y,z) of the
-// tet's local box; each lane walks its row's x-span and builds the row word.
-__device__ __forceinline__ void raster_fast(const int* rec, u32* img, int lane, int img_stride) {
-    const u32 box = (u32)rec[16];
-    const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
-    const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
-    const int w = x1 - x0 + 1, ny = y1 - y0 + 1, nrows = ny * (z1 - z0 + 1);
-    const int n4 = (w + 3) & ~3;  // samples walked: x0+n4-1 down to x0
-    const int4 MX = *reinterpret_cast<const int4*>(rec);
-    const int4 MY = *reinterpret_cast<const int4*>(rec + 4);
-    const int4 MZ = *reinterpret_cast<const int4*>(rec + 8);
-    const int4 G0 = *reinterpret_cast<const int4*>(rec + 12);
-    const int xs = x0 + n4 - 1;
-    // unsigned arithmetic: positions beyond x=31 may wrap; their bits are masked off below
-    const u32 e0 = (u32)G0.x + (u32)MX.x * (u32)xs, e1 = (u32)G0.y + (u32)MX.y * (u32)xs;
-    const u32 e2 = (u32)G0.z + (u32)MX.z * (u32)xs, e3 = (u32)G0.w + (u32)MX.w * (u32)xs;
-    const u32 wmask = 0xFFFFFFFFu >> (32 - w);
-    const u32 inv = (65536u + ny - 1) / ny;  // r / ny for r < 1024, ny <= 32 (checked in tests)
-    for (int r = lane; r < nrows; r += 32) {
-        const int zz = (int)(((u32)r * inv) >> 16);
-        const int y = y0 + (r - zz * ny), z = z0 + zz;
-        u32 r0 = e0 + (u32)MY.x * (u32)y + (u32)MZ.x * (u32)z;
-        u32 r1 = e1 + (u32)MY.y * (u32)y + (u32)MZ.y * (u32)z;
-        u32 r2 = e2 + (u32)MY.z * (u32)y + (u32)MZ.z * (u32)z;
-        u32 r3 = e3 + (u32)MY.w * (u32)y + (u32)MZ.w * (u32)z;
-        u32 out = 0;  // bit q = 1 iff sample x0+q is OUTSIDE
-        for (int i = 0; i < n4; i += 4) {
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                out = __funnelshift_l(r0 | r1 | r2 | r3, out, 1);
-                r0 -= (u32)MX.x; r1 -= (u32)MX.y; r2 -= (u32)MX.z; r3 -= (u32)MX.w;
-            }
-        }
-        const u32 word = (~out & wmask) << x0;
-        if (word) atomicOr(img + z * img_stride + y, word);
-    }
-}
-
-// Large path (K5): planes do not fit int32 on this tile.  The whole warp works on one
-// (tet, tile): exact classification of the local box, then a 64-bit ballot rasteriser
-// with lanes = the 32 x positions of a row word.
-__device__ __noinline__ void raster_large(const Params& p, u32 t, u32 box, int X0, int Y0, int Z0, u32* img, int lane,
-                                          int img_stride) {
-    Tet q = load_tet(p, t);
-    Planes P;
-    tet_planes(p, q, X0, Y0, Z0, P);
-    const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
-    const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
-    bool all_in = true, any_out = false;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        i64 ax0 = P.mx[k] * x0, ax1 = P.mx[k] * x1, ay0 = P.my[k] * y0, ay1 = P.my[k] * y1;
-        i64 az0 = P.mz[k] * z0, az1 = P.mz[k] * z1;
-        i64 lo = P.g0[k] + min(ax0, ax1) + min(ay0, ay1) + min(az0, az1);
-        i64 hi = P.g0[k] + max(ax0, ax1) + max(ay0, ay1) + max(az0, az1);
-        all_in = all_in && (lo >= 0);
-        any_out = any_out || (hi < 0);
-    }
-    if (any_out) return;  // one half-space misses the whole box: exact, G is affine
-    const u32 xmask = (0xFFFFFFFFu >> (31 - x1 + x0)) << x0;
-    const int ny = y1 - y0 + 1;
-    if (all_in) {  // the box lies inside the tet
-        const int nrows = ny * (z1 - z0 + 1);
-        for (int r = lane; r < nrows; r += 32) {
-            int zz = r / ny;
-            atomicOr(img + (z0 + zz) * img_stride + y0 + r - zz * ny, xmask);
-        }
-        return;
-    }
-    i64 c0 = P.g0[0] + P.mx[0] * lane, c1 = P.g0[1] + P.mx[1] * lane;
-    i64 c2 = P.g0[2] + P.mx[2] * lane, c3 = P.g0[3] + P.mx[3] * lane;
-    for (int z = z0; z <= z1; ++z) {
-        i64 r0 = c0 + P.mz[0] * z + P.my[0] * y0, r1 = c1 + P.mz[1] * z + P.my[1] * y0;
-        i64 r2 = c2 + P.mz[2] * z + P.my[2] * y0, r3 = c3 + P.mz[3] * z + P.my[3] * y0;
-        for (int y = y0; y <= y1; ++y) {
-            u32 word = __ballot_sync(0xFFFFFFFFu, (r0 | r1 | r2 | r3) >= 0) & xmask;
-            if (lane == 0 && word) atomicOr(img + z * img_stride + y, word);
-            r0 += P.my[0]; r1 += P.my[1]; r2 += P.my[2]; r3 += P.my[3];
-        }
-    }
-}
-
-template <int NT>
-__global__ void __launch_bounds__(NT) k4_brick(Params p, const u32* __restrict__ offsets, const u32* __restrict__ list,
-                                               u32* __restrict__ bits, u32* __restrict__ hdr) {
-    __shared__ u32 img[32 * 43];
-    __shared__ __align__(16) int rec[NT][REC_W + 2];  // row = 20 words: int4-aligned
-    __shared__ u32 s_large;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int NW = NT / 32;
-    const u32 b = blockIdx.x;
-    const u32 bx = b % p.nbx;
-    u32 rest = b / p.nbx;
-    const u32 by = rest % p.nby;
-    rest /= p.nby;
-    const u32 bz = rest % p.nbz;
-    const u32 m = rest / p.nbz;
-    const int X0 = bx << 5, Y0 = by << p.ty_log, Z0 = bz << p.tz_log;
-    const int rows = 1 << (p.ty_log + p.tz_log);
-    const int img_stride = (1 << p.ty_log) + 11;
-    for (int i = tid; i < (img_stride << p.tz_log); i += NT) img[i] = 0;
-    if (tid == 0) s_large = 0;
-    const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
-    for (u32 base = beg; base < end; base += NT) {
-        __syncthreads();
-        const int n = min((u32)NT, end - base);
-        if (tid < n) setup_record(p, list[base + tid], X0, Y0, Z0, rec[tid]);
-        __syncthreads();
-        for (int i = warp; i < n; i += NW) {
-            const int* r = rec[i];
-            if (r[17] == KIND_FAST) {
-                raster_fast(r, img, lane, img_stride);
-            } else {
-                raster_large(p, (u32)r[0], (u32)r[16], X0, Y0, Z0, img, lane, img_stride);
-                if (lane == 0) atomicAdd(&s_large, 1u);
-            }
-        }
-    }
-    __syncthreads();
-    const int TY = 1 << p.ty_log;
-    for (int i = tid; i < rows; i += NT) {
-        const int z = i >> p.ty_log, y = i & (TY - 1);
-        const int gy = Y0 + y, gz = Z0 + z;
-        if (gy < p.ny && gz < p.nz)
-            bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[z * img_stride + y];
-    }
-    if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -894,107 +727,9 @@ __device__ __forceinline__ int span_bound(int r, int mx, int inv) {
     return c0 + (v >> 31);
 }
 
-template <int NLO>
-__device__ __forceinline__ void raster_span(const int* rec, int lane, int img_stride) {
-    const int4 MX = *reinterpret_cast<const int4*>(rec);
-    const int4 MY = *reinterpret_cast<const int4*>(rec + 4);
-    const int4 MZ = *reinterpret_cast<const int4*>(rec + 8);
-    const int4 G0 = *reinterpret_cast<const int4*>(rec + 12);
-    const int4 IV = *reinterpret_cast<const int4*>(rec + 16);
-    const int4 A = *reinterpret_cast<const int4*>(rec + 20);  // x0+1, x1-x0, ny, nrows
-    const int2 B = *reinterpret_cast<const int2*>(rec + 24);  // shared byte address of row (y0,z0), div magic
-    for (int r = lane; r < A.w; r += 32) {
-        const int zz = (int)(((u32)r * (u32)B.y) >> 16);
-        const int yy = r - zz * A.z;
-        const int b0 = span_bound(G0.x + MY.x * yy + MZ.x * zz, MX.x, IV.x);
-        const int b1 = span_bound(G0.y + MY.y * yy + MZ.y * zz, MX.y, IV.y);
-        const int b2 = span_bound(G0.z + MY.z * yy + MZ.z * zz, MX.z, IV.z);
-        const int b3 = span_bound(G0.w + MY.w * yy + MZ.w * zz, MX.w, IV.w);
-        int lower, upper;  // lower = (first solid x) - 1
-        if (NLO == 1) { lower = max(-1, b0); upper = min(min(A.y, b1), min(b2, b3)); }
-        else if (NLO == 2) { lower = max(-1, max(b0, b1)); upper = min(A.y, min(b2, b3)); }
-        else { lower = max(max(-1, b0), max(b1, b2)); upper = min(A.y, b3); }
-        const int n = upper - lower;  // number of solid voxels in the row (<= 0: none)
-        const u32 saddr = (u32)B.x + 4u * (u32)(zz * img_stride + yy);
-        // branch-free: PTX shifts clamp at 32, so n <= 0 gives word 0 and the OR is a no-op
-        asm volatile(
-            "{\n\t.reg .b32 m, s;\n\t"
-            "sub.s32 s, 32, %1;\n\t"
-            "shr.b32 m, 0xFFFFFFFF, s;\n\t"
-            "add.s32 s, %2, %3;\n\t"
-            "shl.b32 m, m, s;\n\t"
-            "red.shared.or.b32 [%0], m;\n\t}"
-            ::"r"(saddr), "r"(n), "r"(lower), "r"(A.x)
-            : "memory");
-    }
-}
-
-// (kept as vox_set_variant 3 for A/B runs and parity: warp per pair, lanes = rows; dense output only)
-template <int NT, int MINB>
-__global__ void __launch_bounds__(NT, MINB) k4_span(Params p, const u32* __restrict__ offsets,
-                                                    const u32* __restrict__ list, u32* __restrict__ bits,
-                                                    u32* __restrict__ hdr) {
-    __shared__ u32 img[32 * (32 + IMG_SKEW)];
-    __shared__ __align__(16) int rec[NT][SREC_W];
-    __shared__ u32 s_large;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int NW = NT / 32;
-    const u32 b = blockIdx.x;
-    const u32 bx = b % p.nbx;
-    u32 rest = b / p.nbx;
-    const u32 by = rest % p.nby;
-    rest /= p.nby;
-    const u32 bz = rest % p.nbz;
-    const u32 m = rest / p.nbz;
-    const int X0 = bx << 5, Y0 = by << p.ty_log, Z0 = bz << p.tz_log;
-    const int TY = 1 << p.ty_log, img_stride = TY + IMG_SKEW;
-    const int img_words = img_stride << p.tz_log;
-    const u32 img_saddr = (u32)__cvta_generic_to_shared(img);
-    for (int i = tid; i < img_words; i += NT) img[i] = 0;
-    if (tid == 0) s_large = 0;
-    const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
-    u32 seen_large = 0;
-    for (u32 base = beg; base < end; base += NT) {
-        __syncthreads();
-        const int n = min((u32)NT, end - base);
-        if (tid < n) {
-            setup_span_record(p, list[base + tid], X0, Y0, Z0, img_stride, img_saddr, rec[tid]);
-            if ((rec[tid][R_INFO] >> 8) != KIND_SPAN) atomicAdd(&s_large, 1u);
-        }
-        __syncthreads();
-        for (int i = warp; i < n; i += NW) {
-            const int* r = rec[i];
-            const int info = r[R_INFO];
-            // nlo == 0 or 4 cannot happen for a non-degenerate tet (the four sigma*N sum to zero
-            // and planes with N_x == 0 count as hi-type); KIND_LARGE (info >= 256) is drawn below
-            if (info == 2) raster_span<2>(r, lane, img_stride);
-            else if (info == 1) raster_span<1>(r, lane, img_stride);
-            else if (info == 3) raster_span<3>(r, lane, img_stride);
-        }
-        // large pairs of this batch (rare): kept out of the loop above so that it holds no call
-        const u32 nl = s_large;  // cumulative; stable between the barrier above and the next one
-        if (nl != seen_large) {
-            seen_large = nl;
-            for (int i = warp; i < n; i += NW) {
-                const int* r = rec[i];
-                if ((r[R_INFO] >> 8) != KIND_SPAN) raster_large_rec(r, img, lane, img_stride);
-            }
-        }
-    }
-    __syncthreads();
-    const int rows = 1 << (p.ty_log + p.tz_log);
-    if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
-    for (int i = tid; i < rows; i += NT) {
-        const int z = i >> p.ty_log, y = i & (TY - 1);
-        const int gy = Y0 + y, gz = Z0 + z;
-        if (gy < p.ny && gz < p.nz)
-            bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[z * img_stride + y];
-    }
-}
-
 // ------------------------------------------------------------------------------------------
 // K4 v3: row-flattened span voxelizer (default).  DESIGN.md "Kernels / K4 flat".
-// Same records and the same exact row-span arithmetic as k4_span, but the rows of a batch of NT
+// The rows of a batch of NT
 // (tet,tile) pairs are laid end to end and dealt out in equal runs: thread i draws rows
 // [i*R, (i+1)*R) of the batch, whichever pairs they belong to, stepping to the next pair's record when
 // one ends.  Every lane is busy whatever the pairs' sizes are (a pair clipped to 9 rows used to occupy a
@@ -1325,7 +1060,7 @@ extern "C" int vox_create(vox_ctx** out, int nx, int ny, int nz, int ex, int ey,
     p.lim_x = ((1 << 30) - 1) / p.sx; p.lim_y = ((1 << 30) - 1) / p.sy; p.lim_z = ((1 << 30) - 1) / p.sz;
     p.wpr = nx / 32;
     auto_tile(p, 0);
-    if ((i64)batch * (nx / 32) * p.nby * p.nbz > 0xFFFFFFF0ll) { free(c); return VOX_ERANGE; }
+    if ((i64)batch * (nx / 32) * p.nby * p.nbz > 0x7FFFFFFFll) { free(c); return VOX_ERANGE; }  // one CTA per tile: gridDim.x
     c->pairs_planned = -1;
     *out = c;
     return VOX_OK;
@@ -1372,13 +1107,15 @@ extern "C" int vox_set_tile(vox_ctx* ctx, int ty, int tz) {
     if (ctx->have_tets) return VOX_ESTATE;
     if (ilog2_exact(ty) < 2 || ty > 32 || ilog2_exact(tz) < 2 || tz > 32) return VOX_EINVAL;
     if ((ctx->p.ny + ty - 1) / ty > 1024 || (ctx->p.nz + tz - 1) / tz > 1024) return VOX_ERANGE;
+    if ((i64)ctx->p.batch * (ctx->p.nx / 32) * ((ctx->p.ny + ty - 1) / ty) * ((ctx->p.nz + tz - 1) / tz) > 0x7FFFFFFFll)
+        return VOX_ERANGE;  // one CTA per tile: gridDim.x
     set_tile(ctx->p, ty, tz);
     ctx->tile_user = true;
     return VOX_OK;
 }
 
 extern "C" int vox_set_variant(vox_ctx* ctx, int variant) {
-    if (!ctx) return VOX_EINVAL;
+    if (!ctx || variant != 0) return VOX_EINVAL;  // no A/B variant is compiled in at present
     ctx->variant = variant;
     return VOX_OK;
 }
@@ -1455,16 +1192,18 @@ static int enqueue_count_scan(vox_ctx* ctx, cudaStream_t st, char* ws, cudaEvent
     if (p.T > 0) {
         unsigned blocks = (unsigned)((p.T + 255) / 256);
         k1_count<<<blocks, 256, 0, st>>>(p, range, counts, hdr, big);
+        count_launch();
     }
     if (ev) CK(cudaEventRecord(ev[1], st));
     k2_scan<<<1, 1024, 0, st>>>(p, range, big, (u32*)(ws + L.list), counts, cursor, hdr, with_list ? 1 : 0);
+    count_launch();
     CK(cudaGetLastError());
     if (ev) CK(cudaEventRecord(ev[2], st));
     return VOX_OK;
 }
 
 extern "C" int vox_plan(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes, int64_t* pairs_out) {
-    if (!ctx || !d_workspace) return VOX_EINVAL;
+    if (!ctx || !d_workspace || ((uintptr_t)d_workspace & 15) != 0) return VOX_EINVAL;
     if (!ctx->have_tets) return VOX_ESTATE;
     WsLayout L = ws_layout(ctx->p);
     if (ws_bytes < L.fixed_end) return VOX_EWORKSPACE;
@@ -1520,6 +1259,7 @@ extern "C" int vox_sparse_status(vox_ctx* ctx, void* cuda_stream, const void* d_
 }
 
 static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes, uint32_t* d_bits_out) {
+    if (((uintptr_t)d_workspace & 15) != 0) return VOX_EINVAL;  // uint2 / uint4 accesses of the workspace arrays
     if (!ctx->have_tets) return VOX_ESTATE;
     Params& p = ctx->p;
     WsLayout L = ws_layout(p);
@@ -1539,15 +1279,15 @@ static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t w
     if (p.T > 0) {
         unsigned blocks = (unsigned)((p.T + 255) / 256);
         k3_scatter<<<blocks, 256, 0, st>>>(p, range, cursor, list, hdr);
+        count_launch();
     }
     if (ev) CK(cudaEventRecord(ev[3], st));
     const SparseOut so = ctx->sparse;
     if (so.table) {
         k4_flat<128, 8, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);
-    } else switch (ctx->variant) {  // A/B variants kept for the parity tests and the history in DESIGN.md
-        case 1: k4_brick<256><<<p.NB, 256, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
-        case 3: k4_span<128, 8><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr); break;
-        default: k4_flat<128, 8, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);  // 64 regs, 32 warps/SM
+        count_launch();
+    } else {
+        k4_flat<128, 8, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);  // 64 regs, 32 warps/SM
     }
     CK(cudaGetLastError());
     if (ev) {
@@ -1574,7 +1314,7 @@ extern "C" int vox_status(vox_ctx* ctx, void* cuda_stream, const void* d_workspa
 }
 
 extern "C" int vox_validate(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes) {
-    if (!ctx || !d_workspace) return VOX_EINVAL;
+    if (!ctx || !d_workspace || ((uintptr_t)d_workspace & 15) != 0) return VOX_EINVAL;
     if (!ctx->have_tets) return VOX_ESTATE;
     Params& p = ctx->p;
     WsLayout L = ws_layout(p);
@@ -1585,6 +1325,7 @@ extern "C" int vox_validate(vox_ctx* ctx, void* cuda_stream, void* d_workspace, 
     i64 n = p.V > p.T ? p.V : p.T;
     if (n < p.batch + 1) n = p.batch + 1;
     k_validate<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, hdr);
+    count_launch();
     CK(cudaGetLastError());
     u32 h[HDR_WORDS];
     CK(cudaMemcpyAsync(h, hdr, sizeof(h), cudaMemcpyDeviceToHost, st));
@@ -1716,10 +1457,10 @@ extern "C" int vox_occupancy(void* cuda_stream, const uint32_t* d_bits_fine, int
     if (total > 0x7FFFFFFFll * 256) return VOX_ERANGE;
     const unsigned blocks = (unsigned)((total + 255) / 256);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (k == 2 && vec) k_occupancy<2, 4><<<blocks, 256, 0, st>>>(d_bits_fine, nx, ny, nz, batch, d_counts_out);
-    else if (k == 2) k_occupancy<2, 1><<<blocks, 256, 0, st>>>(d_bits_fine, nx, ny, nz, batch, d_counts_out);
-    else if (vec) k_occupancy<4, 4><<<blocks, 256, 0, st>>>(d_bits_fine, nx, ny, nz, batch, d_counts_out);
-    else k_occupancy<4, 1><<<blocks, 256, 0, st>>>(d_bits_fine, nx, ny, nz, batch, d_counts_out);
+    if (k == 2 && vec) k_occupancy<2, 4><<<blocks, 256, 0, st>>>(d_bits_fine, nx, ny, nz, batch, d_counts_out), count_launch();
+    else if (k == 2) k_occupancy<2, 1><<<blocks, 256, 0, st>>>(d_bits_fine, nx, ny, nz, batch, d_counts_out), count_launch();
+    else if (vec) k_occupancy<4, 4><<<blocks, 256, 0, st>>>(d_bits_fine, nx, ny, nz, batch, d_counts_out), count_launch();
+    else k_occupancy<4, 1><<<blocks, 256, 0, st>>>(d_bits_fine, nx, ny, nz, batch, d_counts_out), count_launch();
     return cudaGetLastError() == cudaSuccess ? VOX_OK : VOX_ECUDA;
 }
 
@@ -1820,7 +1561,10 @@ extern "C" int vox_pipe_create(vox_pipe** out, int nx, int ny, int nz, int ex, i
 
 extern "C" int vox_pipe_set_variant(vox_pipe* pipe, int variant) {
     if (!pipe) return VOX_EINVAL;
-    for (int i = 0; i < pipe->depth; ++i) vox_set_variant(pipe->slot[i].ctx, variant);
+    for (int i = 0; i < pipe->depth; ++i) {
+        int rc = vox_set_variant(pipe->slot[i].ctx, variant);
+        if (rc) return rc;
+    }
     return VOX_OK;
 }
 
@@ -1923,41 +1667,59 @@ static int pipe_submit(vox_pipe* pipe, const int32_t* h_verts, int64_t V, const 
     }
     const ArenaLayout& A = pipe->A;
     char* a = s.base;
-    // copy-in stream
-    if (V > 0) PCK(cudaMemcpyAsync(a + A.verts, h_verts, (size_t)V * 12, cudaMemcpyHostToDevice, pipe->s_in));
-    if (lat.cx)  // the keep mask (one byte per cell) travels in the slot's tet region
-        PCK(cudaMemcpyAsync(a + A.tets, lat.h_keep, (size_t)(T / 6), cudaMemcpyHostToDevice, pipe->s_in));
-    else if (T > 0) PCK(cudaMemcpyAsync(a + A.tets, h_tets, (size_t)T * 16, cudaMemcpyHostToDevice, pipe->s_in));
-    if (ctx->p.batch > 1 && !lat.cx)
-        PCK(cudaMemcpyAsync(a + A.off, h_tet_offsets, ((size_t)ctx->p.batch + 1) * 8, cudaMemcpyHostToDevice, pipe->s_in));
-    PCK(cudaEventRecord(s.in_done, pipe->s_in));
-    // compute stream
-    PCK(cudaStreamWaitEvent(pipe->s_run, s.in_done, 0));
+    // everything that can be refused is checked BEFORE the first enqueue: the mesh binding (host-side state only)
+    // and the device view of the caller's payload buffer
     int rc = lat.cx ? vox_lattice(ctx, (const int32_t*)(a + A.verts), lat.cx, lat.cy, lat.cz, (const uint8_t*)(a + A.tets))
                     : vox_tets(ctx, (const int32_t*)(a + A.verts), V, (const int32_t*)(a + A.tets), T,
                                (const int64_t*)(a + A.off));
     if (rc) return rc;
+    void* d_payload = NULL;
+    if (cap_tiles > 0) PCK(cudaHostGetDevicePointer(&d_payload, h_payload, 0));
+    // From here on work is in flight on the slot's arena slice: a failure must not return before it has drained
+    // (the next submit would pick the same slot and overwrite the slice under the running copies / kernels).
+#define PCK_DRAIN(call)                                            \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) {                                   \
+            pipe_fail(pipe, e_, #call);                            \
+            cudaStreamSynchronize(pipe->s_in);                     \
+            cudaStreamSynchronize(pipe->s_run);                    \
+            cudaStreamSynchronize(pipe->s_out);                    \
+            return VOX_ECUDA;                                      \
+        }                                                          \
+    } while (0)
+    // copy-in stream
+    if (V > 0) PCK_DRAIN(cudaMemcpyAsync(a + A.verts, h_verts, (size_t)V * 12, cudaMemcpyHostToDevice, pipe->s_in));
+    if (lat.cx)  // the keep mask (one byte per cell) travels in the slot's tet region
+        PCK_DRAIN(cudaMemcpyAsync(a + A.tets, lat.h_keep, (size_t)(T / 6), cudaMemcpyHostToDevice, pipe->s_in));
+    else if (T > 0) PCK_DRAIN(cudaMemcpyAsync(a + A.tets, h_tets, (size_t)T * 16, cudaMemcpyHostToDevice, pipe->s_in));
+    if (ctx->p.batch > 1 && !lat.cx)
+        PCK_DRAIN(cudaMemcpyAsync(a + A.off, h_tet_offsets, ((size_t)ctx->p.batch + 1) * 8, cudaMemcpyHostToDevice, pipe->s_in));
+    PCK_DRAIN(cudaEventRecord(s.in_done, pipe->s_in));
+    // compute stream
+    PCK_DRAIN(cudaStreamWaitEvent(pipe->s_run, s.in_done, 0));
     size_t out_bytes = vox_grid_words(ctx) * 4;
     if (cap_tiles < 0) {
         rc = vox_run(ctx, pipe->s_run, a + A.ws, pipe->slice_bytes - A.ws, (uint32_t*)(a + A.bits));
     } else {
         // the kernel stores mixed tiles straight into the caller's pinned payload buffer (device view of it)
-        void* d_payload = NULL;
-        if (cap_tiles > 0) PCK(cudaHostGetDevicePointer(&d_payload, h_payload, 0));
         rc = vox_run_sparse(ctx, pipe->s_run, a + A.ws, pipe->slice_bytes - A.ws, (uint32_t*)(a + A.bits),
                             (uint32_t*)d_payload, cap_tiles);
         out_bytes = (size_t)ctx->p.NB * 4;  // the tile table lives where the dense grid would
     }
     if (rc) {
         if (rc == VOX_ECUDA) snprintf(pipe->err, sizeof(pipe->err), "%s", ctx->err);
+        cudaStreamSynchronize(pipe->s_in);
+        cudaStreamSynchronize(pipe->s_run);
         return rc;
     }
-    PCK(cudaEventRecord(s.run_done, pipe->s_run));
+    PCK_DRAIN(cudaEventRecord(s.run_done, pipe->s_run));
     // copy-out stream
-    PCK(cudaStreamWaitEvent(pipe->s_out, s.run_done, 0));
-    PCK(cudaMemcpyAsync(h_bits_out, a + A.bits, out_bytes, cudaMemcpyDeviceToHost, pipe->s_out));
-    PCK(cudaMemcpyAsync(s.h_hdr, a + A.ws + ws_layout(ctx->p).hdr, HDR_WORDS * 4, cudaMemcpyDeviceToHost, pipe->s_out));
-    PCK(cudaEventRecord(s.out_done, pipe->s_out));
+    PCK_DRAIN(cudaStreamWaitEvent(pipe->s_out, s.run_done, 0));
+    PCK_DRAIN(cudaMemcpyAsync(h_bits_out, a + A.bits, out_bytes, cudaMemcpyDeviceToHost, pipe->s_out));
+    PCK_DRAIN(cudaMemcpyAsync(s.h_hdr, a + A.ws + ws_layout(ctx->p).hdr, HDR_WORDS * 4, cudaMemcpyDeviceToHost, pipe->s_out));
+    PCK_DRAIN(cudaEventRecord(s.out_done, pipe->s_out));
+#undef PCK_DRAIN
     s.ticket = pipe->next_ticket++;
     if (ticket_out) *ticket_out = s.ticket;
     return VOX_OK;
@@ -1979,13 +1741,15 @@ extern "C" const char* vox_pipe_last_error(const vox_pipe* pipe) { return pipe ?
 extern "C" int vox_probe_int32(void* cuda_stream, int kind, int blocks, int iters, uint32_t* d_sink, double* ops_out) {
     if (blocks <= 0 || iters <= 0 || !d_sink) return VOX_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (kind == 0) k_probe<0><<<blocks, 256, 0, st>>>(iters, d_sink);
-    else if (kind == 1) k_probe<1><<<blocks, 256, 0, st>>>(iters, d_sink);
-    else k_probe<2><<<blocks, 256, 0, st>>>(iters, d_sink);
+    if (kind == 0) k_probe<0><<<blocks, 256, 0, st>>>(iters, d_sink), count_launch();
+    else if (kind == 1) k_probe<1><<<blocks, 256, 0, st>>>(iters, d_sink), count_launch();
+    else k_probe<2><<<blocks, 256, 0, st>>>(iters, d_sink), count_launch();
     if (cudaGetLastError() != cudaSuccess) return VOX_ECUDA;
     if (ops_out) *ops_out = (double)blocks * 256.0 * (double)iters * 64.0;
     return VOX_OK;
 }
+
+extern "C" uint64_t vox_kernel_launches(void) { return __atomic_load_n(&g_launches, __ATOMIC_RELAXED); }
 
 extern "C" const char* vox_strerror(int code) {
     switch (code) {

@@ -75,6 +75,29 @@ def test_create_validates(lib):
     lib.vox_destroy(batch)
 
 
+def test_misaligned_workspace_variant_and_tile_count_limits(lib):
+    c = ctypes.c_void_p()
+    E = 65536
+    assert lib.vox_create(ctypes.byref(c), 64, 64, 64, E, E, E, 1) == 0
+    assert lib.vox_tets(c, ctypes.c_void_p(256), 4, ctypes.c_void_p(256), 0, None) == 0
+    # a workspace that is not 16-byte aligned is refused before anything is enqueued (uint2 / uint4 accesses)
+    assert lib.vox_run(c, None, ctypes.c_void_p(256 + 4), 1 << 20, ctypes.c_void_p(256)) == -1
+    assert lib.vox_plan(c, None, ctypes.c_void_p(256 + 8), 1 << 20, None) == -1
+    assert lib.vox_validate(c, None, ctypes.c_void_p(256 + 4), 1 << 20) == -1
+    # no A/B variant is compiled in: refused, not ignored
+    assert lib.vox_set_variant(c, 0) == 0
+    assert lib.vox_set_variant(c, 3) == -1
+    lib.vox_destroy(c)
+    # one CTA per tile: more than 2^31 - 1 tiles cannot be launched -> VOX_ERANGE at create / set_tile
+    assert lib.vox_create(ctypes.byref(c), 32768, 4096, 4096, E, E, E, 1000) == -2
+    assert not c.value
+    assert lib.vox_create(ctypes.byref(c), 32768, 4096, 4096, E, E, E, 100) == 0
+    assert lib.vox_set_tile(c, 4, 4) == -2
+    assert lib.vox_set_tile(c, 32, 32) == 0
+    lib.vox_destroy(c)
+    assert lib.vox_kernel_launches() == 0 or lib.vox_kernel_launches() > 0   # callable without a device
+
+
 def test_strerror(lib):
     seen = set()
     for code in range(0, -7, -1):

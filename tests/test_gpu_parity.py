@@ -95,12 +95,15 @@ def test_parity_is_tile_independent(name, tile):
     assert_same(gpu_voxelize(m, tile=tile), cpu_voxelize(m), f"{name} tile={tile}")
 
 
-@pytest.mark.parametrize("variant", [1, 3])
-@pytest.mark.parametrize("name", ["cfg1_sphere", "cfg2", "cfg4_small_drop3", "giant128_sphere", "giant256_nojit"])
-def test_parity_kernel_variants(name, variant):
-    # variant 1 = the x-walk voxelizer, 3 = the warp-per-pair span voxelizer, kept for A/B comparison; same bits
-    m = CASES[name]()
-    assert_same(gpu_voxelize(m, variant=variant), cpu_voxelize(m), f"{name} variant={variant}")
+def test_unknown_kernel_variant_is_refused():
+    # no A/B variant is compiled in: a non-zero variant must be refused, never silently ignored (dense or sparse)
+    import paper_2106_01326_b200 as pkg
+
+    with pytest.raises(pkg.VoxError) as ei:
+        pkg.Voxelizer((32, 32, 32), variant=3)
+    assert ei.value.code == -1
+    with pytest.raises(pkg.VoxError):
+        pkg.Pipe((32, 32, 32), depth=1, max_V=4, max_T=1, variant=1)
 
 
 def test_estimated_workspace_path():
