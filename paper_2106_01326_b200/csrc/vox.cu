@@ -40,6 +40,9 @@ struct Params {
     int lim_x, lim_y, lim_z;  // (2^30 - 1) / (h/g): largest |N| component whose scaled coefficient fits
     int g, g_shift;      // gcd of the pitches; log2(g) or -1
     int sx, sy, sz;      // h / g
+    int c4x, c4y, c4z;   // -4 * (h / g): sign and scale of a stored plane coefficient (setup_pair's fast path)
+    int pow2;            // every 2h and g is a power of two: shifts instead of divisions
+    float fit_vol, fit_ax, fit_ay, fit_az;  // setup_pair's int32 fit test: 24/g, 16*sx, 16*sy, 16*sz
     int ty_log, tz_log;  // tile = 32 x (1<<ty_log) x (1<<tz_log) voxels
     int nbx, nby, nbz;   // tiles per axis
     int wpr;             // words per grid row = nx/32
@@ -483,34 +486,57 @@ __device__ __forceinline__ void tet_planes(const Params& p, const Tet& q, int X0
 __device__ __forceinline__ i64 iabs64(i64 v) { return v < 0 ? -v : v; }
 
 
-enum { KIND_LARGE = 1 };
-
-__device__ __forceinline__ u32 pack_box(int x0, int x1, int y0, int y1, int z0, int z1) {
-    return (u32)x0 | ((u32)x1 << 5) | ((u32)y0 << 10) | ((u32)y1 << 15) | ((u32)z0 << 20) | ((u32)z1 << 25);
-}
-
 // ------------------------------------------------------------------------------------------
-// K4 v2: row-span voxelizer (default).  DESIGN.md "Kernels / K4 span".
+// K4: row-span voxelizer.  DESIGN.md "Kernels / K4".
 // Inside a tile row (y,z) every half-space G_k(x) = r_k + mx_k*x >= 0 is a half-line in x, so the
 // row's solid set is ONE interval [lower, upper].  Each plane is stored as a function Q that is
 // non-increasing in x and whose non-negative set {x : Q(x) >= 0} is
 //   hi-type (mx_G < 0): Q = G                     -> x <= b,  b = max{x : G(x) >= 0}
 //   lo-type (mx_G > 0): Q = -G - 1  (G <= -1)     -> x <= b  <=> G(x) < 0, so the half-space is x >= b+1
 //   mx_G == 0:          r' = 64*G + 63, mx = 0 (hi) -> gates the row only (see span_plane)
-// b = floor of the real crossing r/|mx|.  A fixed-point reciprocal PROPOSES c0 = floor(r*inv/2^32), which is
-// B or B+1 for r >= 0 (see span_bound); the INTEGER value Q(c0) decides: b = c0 if Q(c0) >= 0 else c0-1.
-// No floating point at all.  Planes are stored scaled by 4 so that |mx| >= 4 and the
-// reciprocal fits int32; all stored Q(x), x in [-1,32], and r +- mx fit int32 (checked in int64 at setup).
+// b = floor of the real crossing r/|mx|.  A fixed-point reciprocal PROPOSES c0 = floor(r*inv/2^32) >= B, which
+// is B or B+1 whenever B < 2^18 (see span_bound); the INTEGER value Q(c0) decides: b = c0 if Q(c0) >= 0 else c0-1.
+// Planes are stored scaled by 4 so that |mx| >= 4 and the reciprocal fits int32; every row value r of the
+// pair's box and r +- 2*mx fit int32 (guaranteed at setup, see setup_pair / span_plane).
 // ------------------------------------------------------------------------------------------
-enum { SREC_W = 40, KIND_SPAN = 0, IMG_SKEW = 11, R_BOX = 38, R_INFO = 39 };  // record stride 40 words: int4-aligned
-// record words: [0..3] mx  [4..7] my  [8..11] mz  [12..15] g0 (at row y0,z0)  [16..19] ceil(2^32/|mx|)
-//               [20] x0+1  [21] x1-x0  [22] ny  [23] nrows  [24] shared byte address of image row (y0,z0)
-//               [25] div magic  [26] c1  [27] c2 (plane 1 / 2 is lo-type ? +2^30 : -2^30)  [39] nlo | kind<<8
-// large records (kind = KIND_LARGE): see large_record
+// Record of one (tet, tile) pair in shared memory, 40 words:
+//   [0..3]   A = x0+1, x1-x0, ny, nrows          (box-relative: rows (yy,zz) and x' = x - x0 count from the pair's box)
+//   [4..7]   B = shared byte address of image row (y0,z0), div-by-ny magic, c1, c2
+//            (c1 / c2: plane slot 1 / 2 is lo-type ? +2^30 : -2^30;  c1 == 0 marks a LARGE record, B.y = its box)
+//   [8..23]  four plane slots {mx, my, mz, g0 (at the box origin)}, lo-types first: slot 0 is always lo, slot 3 always hi
+//   [24..27] ceil-ish 2^32/|mx| of the four slots
+//   large records: [8..39] the 16 int64 values mx[4], my[4], mz[4], g0[4] of tet_planes (tile-relative)
+// Record pi starts at word pi*40 + 4*(pi/4): the 16-byte pad after every fourth record puts the same 16-byte
+// chunk of eight consecutive records into eight different bank groups (2*pi + pi/4 mod 8 is a bijection on
+// 0..7), so the LDS.128 / STS.128 of lanes that sit in neighbouring records do not conflict (stride 40 alone
+// gave two-way conflicts: profiles/r02a).
 // image: row (y,z) of the tile lives at img[z*(TY+IMG_SKEW) + y] (skew spreads a tet's rows over banks)
+enum { SREC_W = 40, IMG_SKEW = 11 };
+#define REC_WORDS(NT) ((NT) * SREC_W + ((NT) / 4) * 4)
+__device__ __forceinline__ int rec_off(int pi) { return pi * SREC_W + ((pi >> 2) << 2); }
+#define LARGE_W(i) (8 + 2 * (i))
 
-// One plane of the span record.  (nx,ny,nz) = sigma*N (int32, exact), (rx,ry,rz) = Q - P0.
-// G(j) = floor(C/g) - sum_a (sigma*N_a*s_a) j_a, C = sigma*N.(Q-P0)
+// per-CTA constants of the tile
+struct TileGeo {
+    int X0, Y0, Z0;       // voxel index of the tile origin
+    int ymax, zmax;       // last row / slice of the tile that lies inside the grid (tile-local)
+    int p0x, p0y, p0z;    // lattice coordinates of the centre of the tile-origin voxel
+    int img_stride;
+    u32 img_saddr;
+};
+
+__device__ __forceinline__ u32 pack_box(int x0, int x1, int y0, int y1, int z0, int z1) {
+    return (u32)x0 | ((u32)x1 << 5) | ((u32)y0 << 10) | ((u32)y1 << 15) | ((u32)z0 << 20) | ((u32)z1 << 25);
+}
+
+// a record that draws nothing: one row whose upper bound is -2 (plane slots are never looked at: n < 0 whatever they hold)
+__device__ __forceinline__ void null_record(int* rec, u32 img_saddr) {
+    *reinterpret_cast<int4*>(rec) = make_int4(1, -2, 1, 1);
+    *reinterpret_cast<int4*>(rec + 4) = make_int4((int)img_saddr, 0, 1 << 30, -(1 << 30));
+}
+
+// One plane of the span record, general path.  (nx,ny,nz) = sigma*N (int32, exact), (rx,ry,rz) = Q - P0 (P0 = centre
+// of the tile-origin voxel).  G(j) = floor(C/g) - sum_a (sigma*N_a*s_a) j_a, C = sigma*N.(Q-P0)
 // The record is written relative to the pair's local box: row (yy,zz), x' = x - x0, so that the stored
 // values are distances from the BOX (not the tile) origin and small tets stay in int32 on coarse lattices.
 __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, int nx, int ny, int nz, int rx, int ry,
@@ -544,22 +570,16 @@ __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, i
     g0 = (int)((u32)g0 << sh) + ((sh == 6) ? 63 : 0);
     const u32 a = max((u32)(-mx), 4u);  // a valid plane with mx != 0 has |mx| >= 4 after scaling
     const u32 inv = (sh == 6) ? 0x7FFFFFFFu : (0xFFFFFFFFu / a) + 1u;  // in [2^32/a, 2^32/a + 1), < 2^31
-    rec[pos] = mx;
-    rec[4 + pos] = my;
-    rec[8 + pos] = mz;
-    rec[12 + pos] = g0;
-    rec[16 + pos] = (int)inv;
+    *reinterpret_cast<int4*>(rec + 8 + 4 * pos) = make_int4(mx, my, mz, g0);
+    rec[24 + pos] = (int)inv;
     return ok;
 }
 
-// record of a large pair: the 16 int64 values mx[4], my[4], mz[4], g0[4] of tet_planes sit in words 0..19 and
-// 26..37 (LARGE_W); words 20..25 hold a one-row span header that draws nothing (x1' = -2), so that the row
-// walk of k4_flat can step over the pair like over any other; [38] packed local box, [39] kind.
-#define LARGE_W(i) ((i) < 10 ? 2 * (i) : 6 + 2 * (i))
-__device__ __noinline__ void large_record(const Params& p, u32 t, int X0, int Y0, int Z0, u32 img_saddr, int* rec) {
-    const Tet q = load_tet(p, t);  // reloaded here (rare path) so that the caller's copy stays in registers
+// record of a large pair: header A = one row that draws nothing (x1' = -2), so that the row walk of k4_flat steps
+// over the pair like over any other; B = image address, packed local box, 0 (= large), 0; words 8..39 the int64 planes
+__device__ __noinline__ void large_record(const Params& p, const Tet& q, const TileGeo& g, u32 box, int* rec) {
     Planes P;
-    tet_planes(p, q, X0, Y0, Z0, P);
+    tet_planes(p, q, g.X0, g.Y0, g.Z0, P);
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         *reinterpret_cast<i64*>(rec + LARGE_W(k)) = P.mx[k];
@@ -567,7 +587,8 @@ __device__ __noinline__ void large_record(const Params& p, u32 t, int X0, int Y0
         *reinterpret_cast<i64*>(rec + LARGE_W(8 + k)) = P.mz[k];
         *reinterpret_cast<i64*>(rec + LARGE_W(12 + k)) = P.g0[k];
     }
-    rec[20] = 0; rec[21] = -2; rec[22] = 1; rec[23] = 1; rec[24] = (int)img_saddr; rec[25] = 0;
+    *reinterpret_cast<int4*>(rec) = make_int4(0, -2, 1, 1);
+    *reinterpret_cast<int4*>(rec + 4) = make_int4((int)g.img_saddr, (int)box, 0, 0);
 }
 
 // b = max{x in [0,31] : q0 - a*x >= 0}, or -1 if there is none (a > 0).  A float quotient PROPOSES (its error is
@@ -581,7 +602,7 @@ __device__ __forceinline__ int span64_bound(i64 q0, i64 a) {
     return c;
 }
 
-// the same, with the int64 planes already in the pair's shared-memory record (large_record)
+// rasterise one large pair from the int64 planes in its record (large_record): one warp
 __device__ __noinline__ void raster_large_rec(const int* rec, u32* img, int lane, int img_stride) {
     Planes P;
 #pragma unroll
@@ -591,7 +612,7 @@ __device__ __noinline__ void raster_large_rec(const int* rec, u32* img, int lane
         P.mz[k] = *reinterpret_cast<const i64*>(rec + LARGE_W(8 + k));
         P.g0[k] = *reinterpret_cast<const i64*>(rec + LARGE_W(12 + k));
     }
-    const u32 box = (u32)rec[R_BOX];
+    const u32 box = (u32)rec[5];
     const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
     const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
     bool all_in = true, any_out = false;
@@ -648,24 +669,17 @@ __device__ __noinline__ void raster_large_rec(const int* rec, u32* img, int lane
     }
 }
 
-// thread-per-(tet,tile) setup in 32-bit arithmetic.  Needs the tet's lattice bbox extent < 2^15 per
-// axis (all edge components < 2^15, so every cross-product component is < 2^31) and g a power of two;
-// anything else, or plane values that do not fit int32 on the tile, is handed to the int64 large path.
-__device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0, int Y0, int Z0, int img_stride,
-                                                  u32 img_saddr, int* rec) {
-    const Tet q = load_tet(p, t);
+// General setup of one pair (any pitch, any magnitude): 32-bit planes with every value range-checked in int64
+// (span_plane) when the tet's lattice bbox is < 2^15 per axis and g is a power of two; anything else, or plane
+// values that do not fit int32 on the pair's box, goes to the int64 large path.  Out of line: setup_pair's fast
+// path is what nearly every pair of the BASELINE workloads takes.
+__device__ __noinline__ void setup_general(const Params& p, const Tet& q, const TileGeo& g, u32 box, int* rec) {
+    const int x0 = box & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31, z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
+    const int x1 = (box >> 5) & 31;
+    const int ny = y1 - y0 + 1, nz = z1 - z0 + 1, nrows = ny * nz;
     const int lox = min(min(q.ax, q.bx), min(q.cx, q.dx)), hix = max(max(q.ax, q.bx), max(q.cx, q.dx));
     const int loy = min(min(q.ay, q.by), min(q.cy, q.dy)), hiy = max(max(q.ay, q.by), max(q.cy, q.dy));
     const int loz = min(min(q.az, q.bz), min(q.cz, q.dz)), hiz = max(max(q.az, q.bz), max(q.cz, q.dz));
-    // local closed voxel box (same rounding as K1's axis_range), clipped to the tile
-    const int TY = 1 << p.ty_log, TZ = 1 << p.tz_log;
-    int x0 = -floor_div_2h(p.hx - 2 * lox, p.hx, p.qx), x1 = floor_div_2h(2 * hix - p.hx, p.hx, p.qx);
-    int y0 = -floor_div_2h(p.hy - 2 * loy, p.hy, p.qy), y1 = floor_div_2h(2 * hiy - p.hy, p.hy, p.qy);
-    int z0 = -floor_div_2h(p.hz - 2 * loz, p.hz, p.qz), z1 = floor_div_2h(2 * hiz - p.hz, p.hz, p.qz);
-    x0 = max(x0 - X0, 0); x1 = min(min(x1, p.nx - 1) - X0, 31);
-    y0 = max(y0 - Y0, 0); y1 = min(min(y1, p.ny - 1) - Y0, TY - 1);
-    z0 = max(z0 - Z0, 0); z1 = min(min(z1, p.nz - 1) - Z0, TZ - 1);
-    const int ny = y1 - y0 + 1, nrows = ny * (z1 - z0 + 1);
     bool ok = (((hix - lox) | (hiy - loy) | (hiz - loz)) < 32768) && (p.g_shift >= 0);
     int nlo = 0;
     if (ok) {
@@ -678,12 +692,15 @@ __device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0
         const int ndx = uy * vz - uz * vy, ndy = uz * vx - ux * vz, ndz = ux * vy - uy * vx;
         const int nax = (int)((u32)nbx - (u32)ncx + (u32)ndx), nay = (int)((u32)nby - (u32)ncy + (u32)ndy);
         const int naz = (int)((u32)nbz - (u32)ncz + (u32)ndz);
-        const i64 det = (i64)ux * nbx + (i64)uy * nby + (i64)uz * nbz;  // 6V = u.(v x w) != 0 (K1 culled 0)
+        const i64 det = (i64)ux * nbx + (i64)uy * nby + (i64)uz * nbz;  // 6V = u.(v x w)
+        if (det == 0) {  // degenerate (G2): contributes nothing.  (K1 culls these; the fused lattice path meets them here)
+            null_record(rec, g.img_saddr);
+            return;
+        }
         const int s = det > 0 ? 1 : -1;
         // sigma = (s, -s, s, -s): F = (s*D_a, -s*D_b, s*D_c, -s*D_d) >= 0 inside
-        const int p0x = p.hx * X0 + (p.hx >> 1), p0y = p.hy * Y0 + (p.hy >> 1), p0z = p.hz * Z0 + (p.hz >> 1);
-        const int arx = q.ax - p0x, ary = q.ay - p0y, arz = q.az - p0z;
-        const int brx = q.bx - p0x, bry = q.by - p0y, brz = q.bz - p0z;
+        const int arx = q.ax - g.p0x, ary = q.ay - g.p0y, arz = q.az - g.p0z;
+        const int brx = q.bx - g.p0x, bry = q.by - g.p0y, brz = q.bz - g.p0z;
         // m_x = -sigma*N_x*sx > 0  <=>  lo-type
         const bool l0 = s * nax < 0, l1 = s * nbx > 0, l2 = s * ncx < 0, l3 = s * ndx > 0;
         nlo = (int)l0 + (int)l1 + (int)l2 + (int)l3;
@@ -691,36 +708,151 @@ __device__ __forceinline__ void setup_span_record(const Params& p, u32 t, int X0
         const int pos1 = l1 ? (int)l0 : nlo + (int)!l0;
         const int pos2 = l2 ? (int)l0 + (int)l1 : nlo + (int)!l0 + (int)!l1;
         const int pos3 = l3 ? nlo - 1 : 3;
-        ok = span_plane(p, rec, pos0, s * nax, s * nay, s * naz, brx, bry, brz, x0, y0, z0, ny, z1 - z0 + 1) && ok;
-        ok = span_plane(p, rec, pos1, -s * nbx, -s * nby, -s * nbz, arx, ary, arz, x0, y0, z0, ny, z1 - z0 + 1) && ok;
-        ok = span_plane(p, rec, pos2, s * ncx, s * ncy, s * ncz, arx, ary, arz, x0, y0, z0, ny, z1 - z0 + 1) && ok;
-        ok = span_plane(p, rec, pos3, -s * ndx, -s * ndy, -s * ndz, arx, ary, arz, x0, y0, z0, ny, z1 - z0 + 1) && ok;
+        ok = span_plane(p, rec, pos0, s * nax, s * nay, s * naz, brx, bry, brz, x0, y0, z0, ny, nz) && ok;
+        ok = span_plane(p, rec, pos1, -s * nbx, -s * nby, -s * nbz, arx, ary, arz, x0, y0, z0, ny, nz) && ok;
+        ok = span_plane(p, rec, pos2, s * ncx, s * ncy, s * ncz, arx, ary, arz, x0, y0, z0, ny, nz) && ok;
+        ok = span_plane(p, rec, pos3, -s * ndx, -s * ndy, -s * ndz, arx, ary, arz, x0, y0, z0, ny, nz) && ok;
     }
     if (!ok) {  // int64 planes for the large path, computed here (one thread per pair) rather than by a whole warp
-        large_record(p, t, X0, Y0, Z0, img_saddr, rec);
-        rec[R_BOX] = (int)pack_box(x0, x1, y0, y1, z0, z1);
-        rec[R_INFO] = KIND_LARGE << 8;
+        if (six_volume(q) == 0) {
+            null_record(rec, g.img_saddr);
+            return;
+        }
+        large_record(p, q, g, box, rec);
         return;
     }
     // nlo == 0 or 4 cannot happen for a non-degenerate tet (the four sigma*N sum to zero and planes with
     // N_x == 0 count as hi-type); such a record is made to draw nothing: one row, x1' = -2
     const bool valid = nlo >= 1 && nlo <= 3;
-    int4 a;
-    a.x = x0 + 1; a.y = valid ? x1 - x0 : -2; a.z = ny; a.w = valid ? nrows : 1;  // shift of the row word, box-relative x1
-    *reinterpret_cast<int4*>(rec + 20) = a;
-    int4 b;
-    b.x = (int)(img_saddr + 4u * (u32)(z0 * img_stride + y0));
-    b.y = (int)((65536u + ny - 1) / ny);
-    b.z = nlo >= 2 ? (1 << 30) : -(1 << 30);   // c1
-    b.w = nlo == 3 ? (1 << 30) : -(1 << 30);   // c2
-    *reinterpret_cast<int4*>(rec + 24) = b;
-    rec[R_INFO] = nlo | (KIND_SPAN << 8);
+    *reinterpret_cast<int4*>(rec) = make_int4(x0 + 1, valid ? x1 - x0 : -2, ny, valid ? nrows : 1);
+    *reinterpret_cast<int4*>(rec + 4) =
+        make_int4((int)(g.img_saddr + 4u * (u32)(z0 * g.img_stride + y0)), (int)((65536u + ny - 1) / ny),
+                  nlo >= 2 ? (1 << 30) : -(1 << 30), nlo == 3 ? (1 << 30) : -(1 << 30));
 }
 
-// b = max{x : Q(x) >= 0} for Q(x) = r + mx*x, mx < 0, whenever r >= 0; some b <= -1 when r < 0.
-// c0 = floor(r * inv / 2^32) with inv in [2^32/|mx|, 2^32/|mx| + 1) and |r| < 2^31 lies in
-// {B, B+1} (B = floor(r/|mx|)) for r >= 0 and is <= -1 for r < 0; the INTEGER value Q(c0) decides.
-// |mx*c0| <= |r| + |mx| < 2^31 (checked at setup), so nothing wraps.
+// inv in [2^32/a, (2^32/a)(1 + 2^-19) + 1) for 4 <= a < 2^31, never below 2^32/a: a (rounded DOWN to float) through
+// rcp.approx (relative error <= 2^-23) times 2^32 (1 + 2^-20), rounded up.  span_bound only needs "not below, and
+// relatively within 2^-18" (see there); a wrong bit cannot come from here, the integer check decides.
+__device__ __forceinline__ int recip_up(u32 a) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(__uint2float_rd(a)));
+    return (int)__float2uint_ru(r * 4294971392.0f);  // 2^32 + 2^12
+}
+
+// One plane of the FAST path.  N = the face normal as Theorem 1 orders it (not yet signed), sig = +-1 its sign
+// sigma, (rx,ry,rz) = Q - P with P the centre of the box-origin voxel.  With t = sign(N_x) != 0:
+//   hi-type <=> sigma*N_x > 0 <=> t == sigma;  stored m = -sigma*N*s (hi) = +sigma*N*s (lo) = -t*N*s in both cases;
+//   W = t*N.(Q-P):  Q0 = floor(W/g) (hi: G itself)  or  -floor(-W/g) - 1 = floor((W-1)/g) (lo: -G - 1).
+// c4 = -4*s_a folds the sign and the scale by 4 into the pitch ratio.  All values fit int32 (setup_pair's test).
+__device__ __forceinline__ void fast_plane(const Params& p, int* rec, int pos, bool lo, int nx, int ny, int nz, int rx,
+                                           int ry, int rz) {
+    const int t = (nx >> 31) | 1;
+    const int ax = abs(nx), by = ny * t, bz = nz * t;
+    const i64 W = (i64)ax * rx + (i64)by * ry + (i64)bz * rz - (lo ? 1 : 0);
+    const int q0 = (int)(W >> p.g_shift);
+    const int mx = ax * p.c4x;  // <= -4
+    *reinterpret_cast<int4*>(rec + 8 + 4 * pos) = make_int4(mx, by * p.c4y, bz * p.c4z, q0 << 2);
+    rec[24 + pos] = recip_up((u32)(-mx));
+}
+
+// closed voxel-index range of the centres h*i + h/2 inside [lo, hi]  (not clamped)
+template <bool POW2>
+__device__ __forceinline__ void centre_range(int lo, int hi, int h, int sh, int& i0, int& i1) {
+    if (POW2) {
+        i0 = -((h - 2 * lo) >> sh);  // ceil((2lo - h) / 2h)
+        i1 = (2 * hi - h) >> sh;
+    } else {
+        i0 = -floor_div_i(h - 2 * lo, 2 * h);
+        i1 = floor_div_i(2 * hi - h, 2 * h);
+    }
+}
+
+// thread-per-(tet,tile) setup.  The pair's local box (the tet's closed voxel bbox clipped to the tile) comes first;
+// an empty box or a degenerate tet gives a record that draws nothing (the binning passes never produce such pairs,
+// the fused lattice path does).  FAST path (POW2: every pitch and g a power of two): when
+//     24*dx*dy*dz/g + 16*max(dy*dz*sx, dx*dz*sy, dx*dy*sz) < 2*10^9   and   dx,dy,dz < 2^15   (d = lattice bbox extent)
+// every stored value fits int32 with room to spare and no per-plane range check is needed:
+//   |N_x| <= 2 dy dz (etc.), so |m| = 4|N|s <= 8 d d s;  for every sample P of the box (a point of the tet's bbox)
+//   |sigma*N.(Q-P)| <= 6 dx dy dz, so every row value |r| <= 4 (6 dx dy dz / g + 1);  span_bound forms r and r - a*c0
+//   with a*|c0| <= |r| (1 + 2^-18) + a: all below 2^31 under the test (float, evaluated with 7% of slack; it only
+//   picks the path, both paths are exact).
+// Planes with N_x == 0 (row gates) and everything that fails the test take setup_general.
+template <bool POW2>
+__device__ __forceinline__ void setup_pair(const Params& p, const TileGeo& g, int4 id, const int* magic, int* rec) {
+    Tet q;
+    {
+        const int32_t* v = p.verts;
+        q.ax = __ldg(v + 3 * (i64)id.x); q.ay = __ldg(v + 3 * (i64)id.x + 1); q.az = __ldg(v + 3 * (i64)id.x + 2);
+        q.bx = __ldg(v + 3 * (i64)id.y); q.by = __ldg(v + 3 * (i64)id.y + 1); q.bz = __ldg(v + 3 * (i64)id.y + 2);
+        q.cx = __ldg(v + 3 * (i64)id.z); q.cy = __ldg(v + 3 * (i64)id.z + 1); q.cz = __ldg(v + 3 * (i64)id.z + 2);
+        q.dx = __ldg(v + 3 * (i64)id.w); q.dy = __ldg(v + 3 * (i64)id.w + 1); q.dz = __ldg(v + 3 * (i64)id.w + 2);
+    }
+    const int lox = min(min(q.ax, q.bx), min(q.cx, q.dx)), hix = max(max(q.ax, q.bx), max(q.cx, q.dx));
+    const int loy = min(min(q.ay, q.by), min(q.cy, q.dy)), hiy = max(max(q.ay, q.by), max(q.cy, q.dy));
+    const int loz = min(min(q.az, q.bz), min(q.cz, q.dz)), hiz = max(max(q.az, q.bz), max(q.cz, q.dz));
+    int x0, x1, y0, y1, z0, z1;
+    centre_range<POW2>(lox, hix, p.hx, p.qx, x0, x1);
+    centre_range<POW2>(loy, hiy, p.hy, p.qy, y0, y1);
+    centre_range<POW2>(loz, hiz, p.hz, p.qz, z0, z1);
+    x0 = max(x0 - g.X0, 0); x1 = min(x1 - g.X0, 31);  // nx % 32 == 0: the tile's 32 columns lie inside the grid
+    y0 = max(y0 - g.Y0, 0); y1 = min(y1 - g.Y0, g.ymax);
+    z0 = max(z0 - g.Z0, 0); z1 = min(z1 - g.Z0, g.zmax);
+    if ((x0 > x1) | (y0 > y1) | (z0 > z1)) {
+        null_record(rec, g.img_saddr);
+        return;
+    }
+    const int dx = hix - lox, dy = hiy - loy, dz = hiz - loz;
+    bool fast = POW2 && ((dx | dy | dz) < 32768);
+    if (fast) {
+        const float fx = (float)dx, fy = (float)dy, fz = (float)dz;
+        const float fyz = fy * fz;
+        fast = fx * fyz * p.fit_vol + fmaxf(fmaxf(fyz * p.fit_ax, fx * fz * p.fit_ay), fx * fy * p.fit_az) < 2.0e9f;
+    }
+    if (fast) {
+        const int ux = q.bx - q.ax, uy = q.by - q.ay, uz = q.bz - q.az;
+        const int vx = q.cx - q.ax, vy = q.cy - q.ay, vz = q.cz - q.az;
+        const int wx = q.dx - q.ax, wy = q.dy - q.ay, wz = q.dz - q.az;
+        // N_b = v x w, N_c = u x w, N_d = u x v, N_a = (v-u) x (w-u) = N_b - N_c + N_d   (all < 2^31: d < 2^15)
+        const int nbx = vy * wz - vz * wy, nby = vz * wx - vx * wz, nbz = vx * wy - vy * wx;
+        const int ncx = uy * wz - uz * wy, ncy = uz * wx - ux * wz, ncz = ux * wy - uy * wx;
+        const int ndx = uy * vz - uz * vy, ndy = uz * vx - ux * vz, ndz = ux * vy - uy * vx;
+        const int nax = nbx - ncx + ndx, nay = nby - ncy + ndy, naz = nbz - ncz + ndz;
+        const i64 det = (i64)ux * nbx + (i64)uy * nby + (i64)uz * nbz;  // 6V = u.(v x w)
+        if (det == 0) {  // degenerate (G2): contributes nothing
+            null_record(rec, g.img_saddr);
+            return;
+        }
+        if ((nax != 0) & (nbx != 0) & (ncx != 0) & (ndx != 0)) {
+            const int s = det > 0 ? 1 : -1;
+            // sigma = (s, -s, s, -s);  lo-type <=> sign(N_x) != sigma
+            const bool l0 = (nax ^ s) < 0, l1 = (nbx ^ s) >= 0, l2 = (ncx ^ s) < 0, l3 = (ndx ^ s) >= 0;
+            const int nlo = (int)l0 + (int)l1 + (int)l2 + (int)l3;  // 1..3: the four sigma*N sum to zero
+            const int pos0 = l0 ? 0 : nlo;
+            const int pos1 = l1 ? (int)l0 : nlo + (int)!l0;
+            const int pos2 = l2 ? (int)l0 + (int)l1 : nlo + (int)!l0 + (int)!l1;
+            const int pos3 = l3 ? nlo - 1 : 3;
+            // Q - P, P = centre of the box-origin voxel;  B - P = (A - P) + u
+            const int arx = q.ax - g.p0x - p.hx * x0, ary = q.ay - g.p0y - p.hy * y0, arz = q.az - g.p0z - p.hz * z0;
+            fast_plane(p, rec, pos0, l0, nax, nay, naz, arx + ux, ary + uy, arz + uz);
+            fast_plane(p, rec, pos1, l1, nbx, nby, nbz, arx, ary, arz);
+            fast_plane(p, rec, pos2, l2, ncx, ncy, ncz, arx, ary, arz);
+            fast_plane(p, rec, pos3, l3, ndx, ndy, ndz, arx, ary, arz);
+            const int ny = y1 - y0 + 1;
+            *reinterpret_cast<int4*>(rec) = make_int4(x0 + 1, x1 - x0, ny, ny * (z1 - z0 + 1));
+            *reinterpret_cast<int4*>(rec + 4) =
+                make_int4((int)(g.img_saddr + 4u * (u32)(z0 * g.img_stride + y0)), magic[ny],
+                          nlo >= 2 ? (1 << 30) : -(1 << 30), nlo == 3 ? (1 << 30) : -(1 << 30));
+            return;
+        }
+    }
+    setup_general(p, q, g, pack_box(x0, x1, y0, y1, z0, z1), rec);
+}
+
+// b = max{x : Q(x) >= 0} for Q(x) = r - a*x (mx = -a, a >= 4), whenever 0 <= r and that b is below 2^18; some value
+// >= 2^18 - 1 when it is not (such a bound does not bind: x' <= 31); some b <= -1 when r < 0.
+// inv in [2^32/a, (2^32/a)(1 + 2^-19) + 1) (exact ceil from span_plane, or recip_up): c0 = floor(r*inv/2^32) >= B =
+// floor(r/a), and c0 <= B + 1 when r/a < 2^18 (the excess is below r/a * 2^-19 + r/2^32 < 1); for r < 0, c0 <= -1.
+// The INTEGER value Q(c0) decides.  |a*c0| <= |r| (1 + 2^-18) + a < 2^31 (guaranteed at setup), so nothing wraps.
 __device__ __forceinline__ int span_bound(int r, int mx, int inv) {
     const int c0 = __mulhi(r, inv);
     const int v = r + mx * c0;
@@ -728,49 +860,44 @@ __device__ __forceinline__ int span_bound(int r, int mx, int inv) {
 }
 
 // ------------------------------------------------------------------------------------------
-// K4 v3: row-flattened span voxelizer (default).  DESIGN.md "Kernels / K4 flat".
-// The rows of a batch of NT
-// (tet,tile) pairs are laid end to end and dealt out in equal runs: thread i draws rows
-// [i*R, (i+1)*R) of the batch, whichever pairs they belong to, stepping to the next pair's record when
-// one ends.  Every lane is busy whatever the pairs' sizes are (a pair clipped to 9 rows used to occupy a
-// whole warp for one pass), and the four warps of the CTA finish together.
+// Row-flattened walk.  The rows of a batch of NT (tet,tile) pairs are laid end to end and dealt out in equal
+// runs: thread i draws rows [i*R, (i+1)*R) of the batch, whichever pairs they belong to, stepping to the next
+// pair's record when one ends.  Every lane is busy whatever the pairs' sizes are (a pair clipped to 9 rows used
+// to occupy a whole warp for one pass), and the four warps of the CTA finish together.
 // ------------------------------------------------------------------------------------------
 struct LaneRec {
-    int4 MX, MY, MZ, G0, IV, A;  // A = x0+1, x1-x0, ny, nrows
-    int saddr, magic;
-    int c1, c2;                  // plane 1 / plane 2 is lo-type ? +2^30 : -2^30
+    int4 A;               // x0+1, x1-x0, ny, nrows
+    int4 B;               // saddr, magic, c1, c2
+    int4 P0, P1, P2, P3;  // plane slots: mx, my, mz, g0
+    int4 IV;
 };
 
 __device__ __forceinline__ void lane_load(const int* rec, LaneRec& L) {
-    L.MX = *reinterpret_cast<const int4*>(rec);
-    L.MY = *reinterpret_cast<const int4*>(rec + 4);
-    L.MZ = *reinterpret_cast<const int4*>(rec + 8);
-    L.G0 = *reinterpret_cast<const int4*>(rec + 12);
-    L.IV = *reinterpret_cast<const int4*>(rec + 16);
-    L.A = *reinterpret_cast<const int4*>(rec + 20);
-    const int4 B = *reinterpret_cast<const int4*>(rec + 24);
-    L.saddr = B.x;
-    L.magic = B.y;
-    L.c1 = B.z;
-    L.c2 = B.w;
+    L.A = *reinterpret_cast<const int4*>(rec);
+    L.B = *reinterpret_cast<const int4*>(rec + 4);
+    L.P0 = *reinterpret_cast<const int4*>(rec + 8);
+    L.P1 = *reinterpret_cast<const int4*>(rec + 12);
+    L.P2 = *reinterpret_cast<const int4*>(rec + 16);
+    L.P3 = *reinterpret_cast<const int4*>(rec + 20);
+    L.IV = *reinterpret_cast<const int4*>(rec + 24);
 }
 
 // one row rr of the pair held in L: the four exact bounds, the span, one OR into the tile image
 __device__ __forceinline__ void lane_row(const LaneRec& L, int rr, int img_stride) {
-    const int zz = (int)(((u32)rr * (u32)L.magic) >> 16);
+    const int zz = (int)(((u32)rr * (u32)L.B.y) >> 16);
     const int yy = rr - zz * L.A.z;
-    const int b0 = span_bound(L.G0.x + L.MY.x * yy + L.MZ.x * zz, L.MX.x, L.IV.x);
-    const int b1 = span_bound(L.G0.y + L.MY.y * yy + L.MZ.y * zz, L.MX.y, L.IV.y);
-    const int b2 = span_bound(L.G0.z + L.MY.z * yy + L.MZ.z * zz, L.MX.z, L.IV.z);
-    const int b3 = span_bound(L.G0.w + L.MY.w * yy + L.MZ.w * zz, L.MX.w, L.IV.w);
-    // planes are stored lo-types first: plane 0 is always lo, plane 3 always hi; |b| <= 2^29
+    const int b0 = span_bound(L.P0.w + L.P0.y * yy + L.P0.z * zz, L.P0.x, L.IV.x);
+    const int b1 = span_bound(L.P1.w + L.P1.y * yy + L.P1.z * zz, L.P1.x, L.IV.y);
+    const int b2 = span_bound(L.P2.w + L.P2.y * yy + L.P2.z * zz, L.P2.x, L.IV.z);
+    const int b3 = span_bound(L.P3.w + L.P3.y * yy + L.P3.z * zz, L.P3.x, L.IV.w);
+    // planes are stored lo-types first: slot 0 is always lo, slot 3 always hi; |b| < 2^30
     // lo-type (c = +2^30): min(b,c) = b joins the lower bounds, max(b,c) = c is no upper bound; hi-type the reverse
-    const int l1 = min(b1, L.c1), u1 = max(b1, L.c1);
-    const int l2 = min(b2, L.c2), u2 = max(b2, L.c2);
+    const int l1 = min(b1, L.B.z), u1 = max(b1, L.B.z);
+    const int l2 = min(b2, L.B.w), u2 = max(b2, L.B.w);
     const int lower = max(max(-1, b0), max(l1, l2));  // (first solid x') - 1, x' = x - x0
     const int upper = min(min(L.A.y, b3), min(u1, u2));
     const int n = upper - lower;
-    const u32 saddr = (u32)L.saddr + 4u * (u32)(zz * img_stride + yy);
+    const u32 saddr = (u32)L.B.x + 4u * (u32)(zz * img_stride + yy);
     // branch-free: PTX shifts clamp at 32, so n <= 0 gives word 0 and the OR is a no-op
     asm volatile(
         "{\n\t.reg .b32 m, s;\n\t"
@@ -836,13 +963,14 @@ __device__ __forceinline__ void tile_epilogue(const Params& p, const u32* img, i
 }
 
 template <int NT, int MINB, bool SPARSE>
-__global__ void __launch_bounds__(NT, MINB) k4_flat(Params p, const u32* __restrict__ offsets,
+__global__ void __launch_bounds__(NT, MINB) k4_flat(const __grid_constant__ Params p, const u32* __restrict__ offsets,
                                                     const u32* __restrict__ list, u32* __restrict__ bits,
-                                                    u32* __restrict__ hdr, SparseOut so) {
+                                                    u32* __restrict__ hdr, const __grid_constant__ SparseOut so) {
     __shared__ u32 img[32 * (32 + IMG_SKEW)];
-    __shared__ __align__(16) int rec[NT][SREC_W];
+    __shared__ __align__(16) int rec[REC_WORDS(NT)];
     __shared__ int s_incl[NT];  // inclusive scan of the pairs' row counts inside each warp's 32 records
     __shared__ int s_wtot[NT / 32];
+    __shared__ int s_magic[33];  // ceil(65536 / ny): row index -> (yy, zz) without a division
     __shared__ u32 s_large;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = NT / 32;
@@ -853,16 +981,23 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(Params p, const u32* __restr
     rest /= p.nby;
     const u32 bz = rest % p.nbz;
     const u32 m = rest / p.nbz;
-    const int X0 = bx << 5, Y0 = by << p.ty_log, Z0 = bz << p.tz_log;
-    const int TY = 1 << p.ty_log, img_stride = TY + IMG_SKEW;
+    const int TY = 1 << p.ty_log, TZ = 1 << p.tz_log;
+    TileGeo g;
+    g.X0 = bx << 5; g.Y0 = by << p.ty_log; g.Z0 = bz << p.tz_log;
+    g.ymax = min(TY, p.ny - g.Y0) - 1;
+    g.zmax = min(TZ, p.nz - g.Z0) - 1;
+    g.p0x = p.hx * g.X0 + (p.hx >> 1); g.p0y = p.hy * g.Y0 + (p.hy >> 1); g.p0z = p.hz * g.Z0 + (p.hz >> 1);
+    g.img_stride = TY + IMG_SKEW;
+    g.img_saddr = (u32)__cvta_generic_to_shared(img);
+    const int img_stride = g.img_stride;
     const int img_words = img_stride << p.tz_log;
-    const u32 img_saddr = (u32)__cvta_generic_to_shared(img);
     const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
     if (SPARSE && beg >= end) {  // no tets: empty tile, nothing else to do
         if (tid == 0) so.table[b] = TILE_EMPTY;
         return;
     }
     for (int i = tid; i < img_words; i += NT) img[i] = 0;
+    if (tid < 33) s_magic[tid] = tid ? (65535 + tid) / tid : 0;
     if (tid == 0) s_large = 0;
     u32 seen_large = 0;
     for (u32 base = beg; base < end; base += NT) {
@@ -870,9 +1005,13 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(Params p, const u32* __restr
         const int n = min((u32)NT, end - base);
         int nr = 0;
         if (tid < n) {
-            setup_span_record(p, list[base + tid], X0, Y0, Z0, img_stride, img_saddr, rec[tid]);
-            if ((rec[tid][R_INFO] >> 8) != KIND_SPAN) atomicAdd(&s_large, 1u);
-            nr = rec[tid][23];  // >= 1 for every pair: large pairs carry a one-row header that draws nothing
+            int* r = rec + rec_off(tid);
+            const u32 t = list[base + tid];
+            const int4 id = p.lcx ? lattice_ids(p, t) : __ldg(p.tets + t);
+            if (p.pow2) setup_pair<true>(p, g, id, s_magic, r);
+            else setup_pair<false>(p, g, id, s_magic, r);
+            if (r[6] == 0) atomicAdd(&s_large, 1u);
+            nr = r[3];  // >= 1 for every pair: large pairs carry a one-row header that draws nothing
         }
         int incl = nr;
 #pragma unroll
@@ -906,12 +1045,13 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(Params p, const u32* __restr
             int pi = w * 32 + j;
             int rr = local - (j ? inc[j - 1] : 0);
             LaneRec L;
-            lane_load(rec[pi], L);
+            lane_load(rec + rec_off(pi), L);
             for (;;) {
                 lane_row(L, rr, img_stride);
                 if (--cnt == 0) break;
                 if (++rr == L.A.w) {  // next pair (every pair has at least one row)
-                    lane_load(rec[++pi], L);
+                    ++pi;
+                    lane_load(rec + rec_off(pi), L);
                     rr = 0;
                 }
             }
@@ -921,14 +1061,14 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(Params p, const u32* __restr
         if (nl != seen_large) {
             seen_large = nl;
             for (int i = warp; i < n; i += NW) {
-                const int* r = rec[i];
-                if ((r[R_INFO] >> 8) != KIND_SPAN) raster_large_rec(r, img, lane, img_stride);
+                const int* r = rec + rec_off(i);
+                if (r[6] == 0) raster_large_rec(r, img, lane, img_stride);
             }
         }
     }
     __syncthreads();
     if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
-    tile_epilogue<NT, SPARSE>(p, img, img_stride, b, bx, m, Y0, Z0, bits, hdr, so, tid);
+    tile_epilogue<NT, SPARSE>(p, img, img_stride, b, bx, m, g.Y0, g.Z0, bits, hdr, so, tid);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1058,6 +1198,9 @@ extern "C" int vox_create(vox_ctx** out, int nx, int ny, int nz, int ex, int ey,
     p.g_shift = ilog2_exact(p.g);
     p.sx = p.hx / p.g; p.sy = p.hy / p.g; p.sz = p.hz / p.g;
     p.lim_x = ((1 << 30) - 1) / p.sx; p.lim_y = ((1 << 30) - 1) / p.sy; p.lim_z = ((1 << 30) - 1) / p.sz;
+    p.c4x = -4 * p.sx; p.c4y = -4 * p.sy; p.c4z = -4 * p.sz;
+    p.pow2 = (p.qx >= 0 && p.qy >= 0 && p.qz >= 0 && p.g_shift >= 0) ? 1 : 0;
+    p.fit_vol = 24.0f / (float)p.g; p.fit_ax = 16.0f * p.sx; p.fit_ay = 16.0f * p.sy; p.fit_az = 16.0f * p.sz;
     p.wpr = nx / 32;
     auto_tile(p, 0);
     if ((i64)batch * (nx / 32) * p.nby * p.nbz > 0x7FFFFFFFll) { free(c); return VOX_ERANGE; }  // one CTA per tile: gridDim.x
@@ -1288,6 +1431,7 @@ static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t w
         count_launch();
     } else {
         k4_flat<128, 8, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);  // 64 regs, 32 warps/SM
+        count_launch();
     }
     CK(cudaGetLastError());
     if (ev) {
