@@ -443,52 +443,74 @@ def run_b200(args):
                 cells = m.cells
                 hk = torch.from_numpy(_mg.lattice_form(m, cells)).pin_memory()
                 lat_T = m.batch * 6 * cells[0] * cells[1] * cells[2]
-                # the implicit tet count picks its own tile: plan once for the exact pair count (outside the timing)
-                vzl = pkg.Voxelizer(m.grid, m.extent, m.batch, tile=args.tile, variant=args.variant)
                 d_keep = hk.cuda()
-                vzl.set_lattice(d_verts, cells, d_keep)
-                lat_pairs = vzl.plan(stream)
-                vzl.run(stream=stream)
-                lat_cap = max(int(vzl.status(stream)["nonempty_tiles"]), 1)  # its tiles differ from the tet-array run's
-                vzl.close()
-                del d_keep
-                lpipe = pkg.Pipe(m.grid, m.extent, m.batch, depth=depth, max_V=m.V, max_T=lat_T, tile=args.tile,
-                                 variant=args.variant, max_pairs=lat_pairs)
-                lts = lpipe.tile_shape
-                lnb = m.batch * lts["nbx"] * lts["nby"] * lts["nbz"]
-                ltabs = [torch.zeros(lnb, dtype=torch.int32).pin_memory() for _ in range(depth)]
-                lpays = [torch.zeros((lat_cap, lts["tz"], lts["ty"]), dtype=torch.int32).pin_memory()
-                         for _ in range(depth)]
-
-                def lat_steps(k, sparse_out):
-                    tickets, last = [], None
-                    for i in range(k):
-                        if i >= depth:
-                            lpipe.wait(tickets[i - depth])
-                        if sparse_out:
-                            tickets.append(lpipe.submit_lattice(hv, cells, hk, ltabs[i % depth], lpays[i % depth], lat_cap))
-                        else:
-                            tickets.append(lpipe.submit_lattice(hv, cells, hk, houts[i % depth]))
-                    for t in tickets[max(0, k - depth):]:
-                        last = lpipe.wait(t)
-                    return last
-
-                res = {}
-                for key, sp in (("dense", False), ("sparse", True)):
-                    lat_steps(max(3, depth), sp)
-                    torch.cuda.synchronize()
-                    t0 = time.perf_counter()
-                    lst = lat_steps(args.e2e_steps, sp)
-                    torch.cuda.synchronize()
-                    lms = (time.perf_counter() - t0) * 1e3
-                    res[key] = {"value": ssum * args.e2e_steps / (lms * 1e-3) / 1e9, "ms_per_step": lms / args.e2e_steps}
-                same_l = bool(torch.equal(houts[0], out.cpu()))
                 e2e_lattice = {"unit": UNIT, "h2d_bytes_per_step": hv.numel() * 4 + hk.numel(), "cells": list(cells),
-                               "dense_output": res["dense"], "sparse_output": res["sparse"], "same_result": same_l,
-                               "pairs": lst["pairs"],
-                               "api": f"vox_pipe_submit_lattice/vox_pipe_wait, depth {depth}"}
-                lpipe.close()
-                del ltabs, lpays
+                               "api": f"vox_pipe_submit_lattice/vox_pipe_wait, depth {depth}",
+                               "paths": "fused = vox_lattice's default (K0 slabs + K4 enumerating its candidate cells, no "
+                                        "K1-K3, no pair list); binned = vox_set_variant(1), the same input through K1-K3"}
+                for path, lvar in (("fused", 0), ("binned", 1)):
+                    # device step of this path on resident inputs (its own tile: the implicit tet count picks it);
+                    # the plan gives the binned path's exact pair count (outside the timing)
+                    vzl = pkg.Voxelizer(m.grid, m.extent, m.batch, tile=args.tile, variant=lvar)
+                    vzl.set_lattice(d_verts, cells, d_keep)
+                    lat_pairs = vzl.plan(stream)
+                    lout = torch.empty_like(out)
+                    for _ in range(3):
+                        vzl.run(lout, stream)
+                    l0, l1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    l0.record(stream)
+                    for _ in range(10):
+                        vzl.run(lout, stream)
+                    l1.record(stream)
+                    stream.synchronize()
+                    lat_dev_ms = l0.elapsed_time(l1) / 10
+                    lst0 = vzl.status(stream)
+                    lat_cap = max(int(lst0["nonempty_tiles"]), 1)
+                    ltile = vzl.tile_shape
+                    lat_ws = vzl.workspace_bytes
+                    same_dev = bool(torch.equal(lout, out))
+                    vzl.close()
+                    del lout
+                    lpipe = pkg.Pipe(m.grid, m.extent, m.batch, depth=depth, max_V=m.V, max_T=lat_T,
+                                     tile=(ltile["ty"], ltile["tz"]), variant=lvar, max_pairs=lat_pairs)
+                    lts = lpipe.tile_shape
+                    lnb = m.batch * lts["nbx"] * lts["nby"] * lts["nbz"]
+                    ltabs = [torch.zeros(lnb, dtype=torch.int32).pin_memory() for _ in range(depth)]
+                    lpays = [torch.zeros((lat_cap, lts["tz"], lts["ty"]), dtype=torch.int32).pin_memory()
+                             for _ in range(depth)]
+
+                    def lat_steps(k, sparse_out):
+                        tickets, last = [], None
+                        for i in range(k):
+                            if i >= depth:
+                                lpipe.wait(tickets[i - depth])
+                            if sparse_out:
+                                tickets.append(lpipe.submit_lattice(hv, cells, hk, ltabs[i % depth], lpays[i % depth], lat_cap))
+                            else:
+                                tickets.append(lpipe.submit_lattice(hv, cells, hk, houts[i % depth]))
+                        for t in tickets[max(0, k - depth):]:
+                            last = lpipe.wait(t)
+                        return last
+
+                    res = {}
+                    for key, sp in (("dense", False), ("sparse", True)):
+                        lat_steps(max(3, depth), sp)
+                        torch.cuda.synchronize()
+                        t0 = time.perf_counter()
+                        lst = lat_steps(args.e2e_steps, sp)
+                        torch.cuda.synchronize()
+                        lms = (time.perf_counter() - t0) * 1e3
+                        res[key] = {"value": ssum * args.e2e_steps / (lms * 1e-3) / 1e9, "ms_per_step": lms / args.e2e_steps}
+                    lat_steps(1, False)
+                    same_l = bool(torch.equal(houts[0], out.cpu()))
+                    e2e_lattice[path] = {"device_ms_per_step": lat_dev_ms,
+                                         "device_value": float(samples) / (lat_dev_ms * 1e-3) / 1e9,
+                                         "dense_output": res["dense"], "sparse_output": res["sparse"],
+                                         "same_result": bool(same_l and same_dev), "pairs": lst["pairs"],
+                                         "tile": [32, ltile["ty"], ltile["tz"]], "workspace_bytes": lat_ws}
+                    lpipe.close()
+                    del ltabs, lpays
+                del d_keep
             pipe.close()
             del htabs, hpays
             # unpipelined single call

@@ -69,8 +69,10 @@ void vox_destroy(vox_ctx* ctx);
  * result of vox_run does not depend on the tile; vox_tile_shape reports it. */
 int vox_set_tile(vox_ctx* ctx, int ty, int tz);
 
-/* Kernel variant of the brick voxelizer for A/B runs, 0 = default.  Result-neutral by contract.  No alternative
- * is compiled in at present: any non-zero value is refused with VOX_EINVAL (never silently ignored). */
+/* Path variant for A/B runs and cross-checks, 0 = default.  Result-neutral by contract.
+ *   1: lattice input (vox_lattice) goes through the binning passes K1-K3 like a tet array instead of the fused
+ *      lattice path; no effect on explicit tets.
+ * Any other value is refused with VOX_EINVAL (never silently ignored). */
 int vox_set_variant(vox_ctx* ctx, int variant);
 
 /* Borrow the mesh.  d_verts int32[V][3] with coordinates in [0, extent];
@@ -88,8 +90,16 @@ int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const int32_t* d_t
  * walking from the cell's low corner along the axes of the q-th permutation of (x,y,z) in lexicographic order
  * (xyz, xzy, yxz, yzx, zxy, zyx); bit q of d_keep[c] says whether tet q is present.  Equivalent to vox_tets with
  * the 6*cx*cy*cz tets written out (absent ones dropped).  With batch > 1 every mesh has the same lattice dims:
- * mesh m's vertices and keep bytes are the m-th block of d_verts / d_keep.  vox_status counts only present tets
- * as culled. */
+ * mesh m's vertices and keep bytes are the m-th block of d_verts / d_keep.
+ * vox_run on lattice input takes the FUSED path: a pass over the vertices (K0) records, per axis and vertex plane
+ * of the lattice, the coordinate range of the plane; each tile then finds the index box of the cells that can
+ * reach it from those ranges and its own coordinates, enumerates their present tets and voxelizes them -- no
+ * per-tet bbox search, no pair list, no K1/K2/K3 (the exact per-tet box inside the tile kernel keeps the result
+ * the definition's).  Its workspace is the header, 8*(cx+cy+cz+3) bytes per mesh and a 16-byte copy of every vertex
+ * (vox_workspace_bytes);
+ * vox_status then reports culled = 0 (slivers and degenerate tets are skipped per tile, not counted per tet).
+ * Lattices beyond 4096 cells per axis or 2^28 vertices, and vox_set_variant(ctx, 1), take the binning passes
+ * (vox_status then counts only present tets as culled).  vox_plan always runs the binning count. */
 int vox_lattice(vox_ctx* ctx, const int32_t* d_verts, int cx, int cy, int cz, const uint8_t* d_keep);
 
 /* batch * nz * ny * (nx/32) */

@@ -29,6 +29,7 @@ struct Params {
     const int32_t* verts;
     const int4* tets;
     const i64* off;  // device, [batch+1] or NULL
+    const int4* verts4;  // fused lattice path: K0's 16-byte copy of the vertices (x, y, z, 0) in the workspace, else NULL
     const unsigned char* keep;  // lattice input (vox_lattice): bit q of keep[cell] = tet q of the cell is present
     int lcx, lcy, lcz;          // cells per axis of the lattice input; lcx == 0: explicit tets
     i64 T;
@@ -90,13 +91,19 @@ static unsigned long long g_launches = 0;
 static inline void count_launch() { __atomic_fetch_add(&g_launches, 1ull, __ATOMIC_RELAXED); }
 
 struct WsLayout {
-    size_t hdr, counts, cursor, big, range, list, fixed_end;
+    size_t hdr, slab, counts, cursor, big, range, list, fixed_end;
 };
+// lattice input: per mesh 2 * ((cx+1) + (cy+1) + (cz+1)) ints of vertex-plane bounds (k0_slabs), else nothing
+static size_t slab_ints(const Params& p) {
+    return p.lcx ? (size_t)p.batch * 2 * ((size_t)p.lcx + p.lcy + p.lcz + 3) : 0;
+}
 static WsLayout ws_layout(const Params& p) {
     WsLayout L;
     size_t o = 0;
     L.hdr = o;
     o = align256(o + HDR_WORDS * 4);
+    L.slab = o;  // (header, slabs and counts are adjacent: one memset clears them)
+    o = align256(o + slab_ints(p) * 4);
     L.counts = o;
     o = align256(o + ((size_t)p.NB + 1) * 4);
     L.cursor = o;
@@ -673,7 +680,7 @@ __device__ __noinline__ void raster_large_rec(const int* rec, u32* img, int lane
 // (span_plane) when the tet's lattice bbox is < 2^15 per axis and g is a power of two; anything else, or plane
 // values that do not fit int32 on the pair's box, goes to the int64 large path.  Out of line: setup_pair's fast
 // path is what nearly every pair of the BASELINE workloads takes.
-__device__ __noinline__ void setup_general(const Params& p, const Tet& q, const TileGeo& g, u32 box, int* rec) {
+__device__ __noinline__ bool setup_general(const Params& p, const Tet q, const TileGeo& g, u32 box, int* rec) {
     const int x0 = box & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31, z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
     const int x1 = (box >> 5) & 31;
     const int ny = y1 - y0 + 1, nz = z1 - z0 + 1, nrows = ny * nz;
@@ -695,7 +702,7 @@ __device__ __noinline__ void setup_general(const Params& p, const Tet& q, const 
         const i64 det = (i64)ux * nbx + (i64)uy * nby + (i64)uz * nbz;  // 6V = u.(v x w)
         if (det == 0) {  // degenerate (G2): contributes nothing.  (K1 culls these; the fused lattice path meets them here)
             null_record(rec, g.img_saddr);
-            return;
+            return false;
         }
         const int s = det > 0 ? 1 : -1;
         // sigma = (s, -s, s, -s): F = (s*D_a, -s*D_b, s*D_c, -s*D_d) >= 0 inside
@@ -716,10 +723,10 @@ __device__ __noinline__ void setup_general(const Params& p, const Tet& q, const 
     if (!ok) {  // int64 planes for the large path, computed here (one thread per pair) rather than by a whole warp
         if (six_volume(q) == 0) {
             null_record(rec, g.img_saddr);
-            return;
+            return false;
         }
         large_record(p, q, g, box, rec);
-        return;
+        return true;
     }
     // nlo == 0 or 4 cannot happen for a non-degenerate tet (the four sigma*N sum to zero and planes with
     // N_x == 0 count as hi-type); such a record is made to draw nothing: one row, x1' = -2
@@ -728,6 +735,7 @@ __device__ __noinline__ void setup_general(const Params& p, const Tet& q, const 
     *reinterpret_cast<int4*>(rec + 4) =
         make_int4((int)(g.img_saddr + 4u * (u32)(z0 * g.img_stride + y0)), (int)((65536u + ny - 1) / ny),
                   nlo >= 2 ? (1 << 30) : -(1 << 30), nlo == 3 ? (1 << 30) : -(1 << 30));
+    return true;
 }
 
 // inv in [2^32/a, (2^32/a)(1 + 2^-19) + 1) for 4 <= a < 2^31, never below 2^32/a: a (rounded DOWN to float) through
@@ -755,6 +763,11 @@ __device__ __forceinline__ void fast_plane(const Params& p, int* rec, int pos, b
     rec[24 + pos] = recip_up((u32)(-mx));
 }
 
+// M with floor(rr*M / 2^16) == rr / ny for all 0 <= rr < 1024, 1 <= ny <= 32: any M in [2^16/ny, 2^16/ny + 2) will do
+// (the excess rr*(M - 2^16/ny)/2^16 stays below 1/ny); floor(2^16/ny) + 1 is one, and the float quotient cannot miss the
+// floor: 2^16/ny is exact for powers of two and at least 1/32 away from an integer otherwise.
+__device__ __forceinline__ int div_magic(int ny) { return __float2int_rz(__fdividef(65536.0f, (float)ny)) + 1; }
+
 // closed voxel-index range of the centres h*i + h/2 inside [lo, hi]  (not clamped)
 template <bool POW2>
 __device__ __forceinline__ void centre_range(int lo, int hi, int h, int sh, int& i0, int& i1) {
@@ -777,31 +790,55 @@ __device__ __forceinline__ void centre_range(int lo, int hi, int h, int sh, int&
 //   with a*|c0| <= |r| (1 + 2^-18) + a: all below 2^31 under the test (float, evaluated with 7% of slack; it only
 //   picks the path, both paths are exact).
 // Planes with N_x == 0 (row gates) and everything that fails the test take setup_general.
-template <bool POW2>
-__device__ __forceinline__ void setup_pair(const Params& p, const TileGeo& g, int4 id, const int* magic, int* rec) {
+// the four vertices of a tet: one 16-byte load each from K0's packed copy (fused lattice path), else 3 x 4 bytes
+template <bool V4>
+__device__ __forceinline__ Tet gather_tet(const Params& p, int4 id) {
     Tet q;
-    {
+    if (V4) {
+        const int4 a = __ldg(p.verts4 + id.x), b = __ldg(p.verts4 + id.y), c = __ldg(p.verts4 + id.z), d = __ldg(p.verts4 + id.w);
+        q.ax = a.x; q.ay = a.y; q.az = a.z; q.bx = b.x; q.by = b.y; q.bz = b.z;
+        q.cx = c.x; q.cy = c.y; q.cz = c.z; q.dx = d.x; q.dy = d.y; q.dz = d.z;
+    } else {
         const int32_t* v = p.verts;
         q.ax = __ldg(v + 3 * (i64)id.x); q.ay = __ldg(v + 3 * (i64)id.x + 1); q.az = __ldg(v + 3 * (i64)id.x + 2);
         q.bx = __ldg(v + 3 * (i64)id.y); q.by = __ldg(v + 3 * (i64)id.y + 1); q.bz = __ldg(v + 3 * (i64)id.y + 2);
         q.cx = __ldg(v + 3 * (i64)id.z); q.cy = __ldg(v + 3 * (i64)id.z + 1); q.cz = __ldg(v + 3 * (i64)id.z + 2);
         q.dx = __ldg(v + 3 * (i64)id.w); q.dy = __ldg(v + 3 * (i64)id.w + 1); q.dz = __ldg(v + 3 * (i64)id.w + 2);
     }
+    return q;
+}
+
+struct LocalBox {
+    int x0, x1, y0, y1, z0, z1;  // tile-local closed voxel box, empty if any lower bound exceeds its upper bound
+    int dx, dy, dz;              // extent of the tet's lattice bbox
+};
+// the tet's closed voxel bbox (same rounding as K1's axis_range) clipped to the tile
+template <bool POW2>
+__device__ __forceinline__ bool local_box(const Params& p, const TileGeo& g, const Tet& q, LocalBox& B) {
     const int lox = min(min(q.ax, q.bx), min(q.cx, q.dx)), hix = max(max(q.ax, q.bx), max(q.cx, q.dx));
     const int loy = min(min(q.ay, q.by), min(q.cy, q.dy)), hiy = max(max(q.ay, q.by), max(q.cy, q.dy));
     const int loz = min(min(q.az, q.bz), min(q.cz, q.dz)), hiz = max(max(q.az, q.bz), max(q.cz, q.dz));
-    int x0, x1, y0, y1, z0, z1;
-    centre_range<POW2>(lox, hix, p.hx, p.qx, x0, x1);
-    centre_range<POW2>(loy, hiy, p.hy, p.qy, y0, y1);
-    centre_range<POW2>(loz, hiz, p.hz, p.qz, z0, z1);
-    x0 = max(x0 - g.X0, 0); x1 = min(x1 - g.X0, 31);  // nx % 32 == 0: the tile's 32 columns lie inside the grid
-    y0 = max(y0 - g.Y0, 0); y1 = min(y1 - g.Y0, g.ymax);
-    z0 = max(z0 - g.Z0, 0); z1 = min(z1 - g.Z0, g.zmax);
-    if ((x0 > x1) | (y0 > y1) | (z0 > z1)) {
+    centre_range<POW2>(lox, hix, p.hx, p.qx, B.x0, B.x1);
+    centre_range<POW2>(loy, hiy, p.hy, p.qy, B.y0, B.y1);
+    centre_range<POW2>(loz, hiz, p.hz, p.qz, B.z0, B.z1);
+    B.x0 = max(B.x0 - g.X0, 0); B.x1 = min(B.x1 - g.X0, 31);  // nx % 32 == 0: the tile's 32 columns lie inside the grid
+    B.y0 = max(B.y0 - g.Y0, 0); B.y1 = min(B.y1 - g.Y0, g.ymax);
+    B.z0 = max(B.z0 - g.Z0, 0); B.z1 = min(B.z1 - g.Z0, g.zmax);
+    B.dx = hix - lox; B.dy = hiy - loy; B.dz = hiz - loz;
+    return (B.x0 <= B.x1) & (B.y0 <= B.y1) & (B.z0 <= B.z1);
+}
+
+template <bool POW2, bool V4>
+__device__ __forceinline__ bool setup_pair(const Params& p, const TileGeo& g, int4 id, int* rec) {
+    const Tet q = gather_tet<V4>(p, id);
+    LocalBox B;
+    const bool hit = local_box<POW2>(p, g, q, B);
+    const int x0 = B.x0, x1 = B.x1, y0 = B.y0, y1 = B.y1, z0 = B.z0, z1 = B.z1;
+    if (!hit) {
         null_record(rec, g.img_saddr);
-        return;
+        return false;
     }
-    const int dx = hix - lox, dy = hiy - loy, dz = hiz - loz;
+    const int dx = B.dx, dy = B.dy, dz = B.dz;
     bool fast = POW2 && ((dx | dy | dz) < 32768);
     if (fast) {
         const float fx = (float)dx, fy = (float)dy, fz = (float)dz;
@@ -820,7 +857,7 @@ __device__ __forceinline__ void setup_pair(const Params& p, const TileGeo& g, in
         const i64 det = (i64)ux * nbx + (i64)uy * nby + (i64)uz * nbz;  // 6V = u.(v x w)
         if (det == 0) {  // degenerate (G2): contributes nothing
             null_record(rec, g.img_saddr);
-            return;
+            return false;
         }
         if ((nax != 0) & (nbx != 0) & (ncx != 0) & (ndx != 0)) {
             const int s = det > 0 ? 1 : -1;
@@ -840,12 +877,12 @@ __device__ __forceinline__ void setup_pair(const Params& p, const TileGeo& g, in
             const int ny = y1 - y0 + 1;
             *reinterpret_cast<int4*>(rec) = make_int4(x0 + 1, x1 - x0, ny, ny * (z1 - z0 + 1));
             *reinterpret_cast<int4*>(rec + 4) =
-                make_int4((int)(g.img_saddr + 4u * (u32)(z0 * g.img_stride + y0)), magic[ny],
+                make_int4((int)(g.img_saddr + 4u * (u32)(z0 * g.img_stride + y0)), div_magic(ny),
                           nlo >= 2 ? (1 << 30) : -(1 << 30), nlo == 3 ? (1 << 30) : -(1 << 30));
-            return;
+            return true;
         }
     }
-    setup_general(p, q, g, pack_box(x0, x1, y0, y1, z0, z1), rec);
+    return setup_general(p, q, g, pack_box(x0, x1, y0, y1, z0, z1), rec);
 }
 
 // b = max{x : Q(x) >= 0} for Q(x) = r - a*x (mx = -a, a >= 4), whenever 0 <= r and that b is below 2^18; some value
@@ -872,14 +909,21 @@ struct LaneRec {
     int4 IV;
 };
 
-__device__ __forceinline__ void lane_load(const int* rec, LaneRec& L) {
-    L.A = *reinterpret_cast<const int4*>(rec);
-    L.B = *reinterpret_cast<const int4*>(rec + 4);
-    L.P0 = *reinterpret_cast<const int4*>(rec + 8);
-    L.P1 = *reinterpret_cast<const int4*>(rec + 12);
-    L.P2 = *reinterpret_cast<const int4*>(rec + 16);
-    L.P3 = *reinterpret_cast<const int4*>(rec + 20);
-    L.IV = *reinterpret_cast<const int4*>(rec + 24);
+__device__ __forceinline__ int4 lds128(u32 saddr) {
+    int4 v;
+    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(saddr));
+    return v;
+}
+// (by shared-memory byte address: the walk keeps the address of its current record in a register and steps it,
+//  instead of rebuilding it from the record index at every pair boundary)
+__device__ __forceinline__ void lane_load(u32 rec_saddr, LaneRec& L) {
+    L.A = lds128(rec_saddr);
+    L.B = lds128(rec_saddr + 16);
+    L.P0 = lds128(rec_saddr + 32);
+    L.P1 = lds128(rec_saddr + 48);
+    L.P2 = lds128(rec_saddr + 64);
+    L.P3 = lds128(rec_saddr + 80);
+    L.IV = lds128(rec_saddr + 96);
 }
 
 // one row rr of the pair held in L: the four exact bounds, the span, one OR into the tile image
@@ -962,16 +1006,75 @@ __device__ __forceinline__ void tile_epilogue(const Params& p, const u32* img, i
     }
 }
 
-template <int NT, int MINB, bool SPARSE>
+// ------------------------------------------------------------------------------------------
+// K0 (fused lattice path): one pass over the lattice vertices that
+//  (1) records per mesh, axis and vertex plane of the lattice the largest coordinate and the largest
+//      (extent - coordinate) over the plane's vertices.  From these a tile finds the index range of the cells whose
+//      tets can reach it (k4_flat<.., LATTICE>) -- no per-tet bbox search, no pair list;
+//        slab of mesh m: [x: lo'(cx+1) hi(cx+1) | y: lo'(cy+1) hi(cy+1) | z: lo'(cz+1) hi(cz+1)],  lo' = extent - min
+//      (zero-initialised by the memset of the header; coordinates lie in [0, extent], so a plain max suffices);
+//  (2) writes a 16-byte copy (x, y, z, 0) of every vertex: K4 then gathers a vertex with one LDG.128 instead of three
+//      4-byte loads (the gather is what loads the LSU pipe in K4's setup, profiles/r02).
+// One CTA per (x plane i, chunk of y rows, mesh); its warps take the chunk's rows in turn, lanes run along z.
+// x: registers + warp reduce; y: warp reduce per row; z: shared-memory atomics; one global atomicMax per value and CTA.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k0_slabs(const int32_t* __restrict__ verts, int cx, int cy, int cz, int ex, int ey,
+                                                int ez, int jchunk, int* __restrict__ slab, int4* __restrict__ verts4) {
+    extern __shared__ int s_z[];  // [cz+1] lo', [cz+1] hi
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int i = blockIdx.x, m = blockIdx.z;
+    const int j0 = blockIdx.y * jchunk, j1 = min(cy + 1, j0 + jchunk);
+    int* sl = slab + (size_t)m * 2 * (cx + cy + cz + 3);
+    int* xlo = sl, *xhi = sl + cx + 1, *ylo = sl + 2 * (cx + 1), *yhi = ylo + cy + 1, *zlo = ylo + 2 * (cy + 1), *zhi = zlo + cz + 1;
+    for (int k = tid; k < 2 * (cz + 1); k += 256) s_z[k] = 0;
+    __syncthreads();
+    int mxlo = 0, mxhi = 0;
+    for (int j = j0 + warp; j < j1; j += 8) {
+        int mylo = 0, myhi = 0;
+        const size_t v0 = (((size_t)m * (cx + 1) + i) * (cy + 1) + j) * (size_t)(cz + 1);
+        const int32_t* row = verts + 3 * v0;
+        for (int k = lane; k <= cz; k += 32) {
+            const int x = __ldg(row + 3 * k), y = __ldg(row + 3 * k + 1), z = __ldg(row + 3 * k + 2);
+            verts4[v0 + k] = make_int4(x, y, z, 0);
+            mxhi = max(mxhi, x); mxlo = max(mxlo, ex - x);
+            myhi = max(myhi, y); mylo = max(mylo, ey - y);
+            atomicMax(s_z + k, ez - z);
+            atomicMax(s_z + cz + 1 + k, z);
+        }
+        myhi = __reduce_max_sync(0xFFFFFFFFu, myhi);
+        mylo = __reduce_max_sync(0xFFFFFFFFu, mylo);
+        if (lane == 0) { atomicMax(yhi + j, myhi); atomicMax(ylo + j, mylo); }
+    }
+    mxhi = __reduce_max_sync(0xFFFFFFFFu, mxhi);
+    mxlo = __reduce_max_sync(0xFFFFFFFFu, mxlo);
+    if (lane == 0) { atomicMax(xhi + i, mxhi); atomicMax(xlo + i, mxlo); }
+    __syncthreads();
+    for (int k = tid; k <= cz; k += 256) { atomicMax(zlo + k, s_z[k]); atomicMax(zhi + k, s_z[cz + 1 + k]); }
+}
+
+// ------------------------------------------------------------------------------------------
+// K4 kernel.  LATTICE = false: the tile's pairs come from the list the binning passes K1-K3 wrote.
+// LATTICE = true (fused lattice path): the tile enumerates its candidate tets itself.  From K0's slabs each of the
+// first three warps finds, for one axis, the first and last cell whose vertex planes reach the tile's sample
+// centres: every tet that has a sample in the tile lies in that index box (a superset).  The box's cells are dealt
+// to the warps in chunks of 32; a lane whose keep bit is set gathers its tet and takes the exact local box
+// (local_box, the one setup_pair uses): only the tets that really reach the tile enter the warp's queue (ballot
+// compaction), 32 of which are set up per batch on dense lanes.  No K1/K2/K3, no range array, no pair list; the
+// price is the box test of the candidates in the rim of the index box.
+// ------------------------------------------------------------------------------------------
+template <int NT, int MINB, bool SPARSE, bool LATTICE>
 __global__ void __launch_bounds__(NT, MINB) k4_flat(const __grid_constant__ Params p, const u32* __restrict__ offsets,
                                                     const u32* __restrict__ list, u32* __restrict__ bits,
-                                                    u32* __restrict__ hdr, const __grid_constant__ SparseOut so) {
+                                                    u32* __restrict__ hdr, const __grid_constant__ SparseOut so,
+                                                    const int* __restrict__ slab) {
     __shared__ u32 img[32 * (32 + IMG_SKEW)];
     __shared__ __align__(16) int rec[REC_WORDS(NT)];
     __shared__ int s_incl[NT];  // inclusive scan of the pairs' row counts inside each warp's 32 records
     __shared__ int s_wtot[NT / 32];
-    __shared__ int s_magic[33];  // ceil(65536 / ny): row index -> (yy, zz) without a division
     __shared__ u32 s_large;
+    __shared__ u32 s_wq[LATTICE ? NT / 32 : 1][LATTICE ? 64 : 1];  // per-warp queue of kept candidates: v0 << 3 | q
+    __shared__ int s_rng[LATTICE ? 6 : 1];
+    __shared__ u32 s_pairs;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = NT / 32;
     const u32 b = blockIdx.x;
@@ -989,29 +1092,162 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(const __grid_constant__ Para
     g.p0x = p.hx * g.X0 + (p.hx >> 1); g.p0y = p.hy * g.Y0 + (p.hy >> 1); g.p0z = p.hz * g.Z0 + (p.hz >> 1);
     g.img_stride = TY + IMG_SKEW;
     g.img_saddr = (u32)__cvta_generic_to_shared(img);
+    const u32 rec_saddr = (u32)__cvta_generic_to_shared(rec);
     const int img_stride = g.img_stride;
     const int img_words = img_stride << p.tz_log;
-    const u32 beg = offsets[b], end = min(offsets[b + 1], p.cap);
-    if (SPARSE && beg >= end) {  // no tets: empty tile, nothing else to do
-        if (tid == 0) so.table[b] = TILE_EMPTY;
-        return;
+    u32 base = 0, end = 0;
+    // LATTICE: candidate index box [ci0, ci0+ni) x [cj0, cj0+nj) x [ck0, ck0+nk), ncand = 6 * cells
+    int ci0 = 0, cj0 = 0, ck0 = 0, nj = 1, nk = 1, wq_n = 0;
+    u32 ncell = 0, chunk = warp, my_pairs = 0;
+    int grp = 0;  // next group of the current chunk (fill stage)
+    const u32 cell_base = m * (u32)p.lcx, vert_base = m * (u32)(p.lcx + 1);  // (32-bit: cells and vertices are below 2^31)
+    // LATTICE: lane = (cell lane_c of the chunk's five, tet lane_q of the cell's six); tet q walks from the cell's low
+    // corner along the axes of the q-th permutation of (x,y,z), lexicographic: xyz xzy yxz yzx zxy zyx (lattice_ids)
+    const int lane_c = lane / 6, lane_q = lane - 6 * lane_c;
+    const int lat_sy = p.lcz + 1, lat_sx = (p.lcy + 1) * (p.lcz + 1), a123 = lat_sx + lat_sy + 1;
+    const int lane_a1 = (lane_q < 2) ? lat_sx : (lane_q < 4) ? lat_sy : 1;
+    const int lane_a12 = a123 - ((lane_q == 3 || lane_q == 5) ? lat_sx : (lane_q == 1 || lane_q == 4) ? lat_sy : 1);
+    float rnk = 0.f, rnj = 0.f;
+    bool small_box = false;
+    if (!LATTICE) {
+        base = offsets[b];
+        end = min(offsets[b + 1], p.cap);
+        if (SPARSE && base >= end) {  // no tets: empty tile, nothing else to do
+            if (tid == 0) so.table[b] = TILE_EMPTY;
+            return;
+        }
+    } else {
+        if (warp < 3) {
+            const int c = warp == 0 ? p.lcx : warp == 1 ? p.lcy : p.lcz;  // cells along this warp's axis
+            const int* lo = slab + (size_t)m * 2 * (p.lcx + p.lcy + p.lcz + 3) +
+                            (warp == 0 ? 0 : warp == 1 ? 2 * (p.lcx + 1) : 2 * (p.lcx + 1) + 2 * (p.lcy + 1));
+            const int* hi = lo + c + 1;
+            const int E = warp == 0 ? p.ex : warp == 1 ? p.ey : p.ez;
+            // the tile's sample centres along this axis: [clo, chi]
+            const int clo = warp == 0 ? g.p0x : warp == 1 ? g.p0y : g.p0z;
+            const int chi = clo + (warp == 0 ? 31 * p.hx : warp == 1 ? g.ymax * p.hy : g.zmax * p.hz);
+            int first = 0x7FFFFFFF, last = -1;
+            for (int i0 = 0; i0 < c; i0 += 32) {
+                const int i = i0 + lane;
+                bool reach = false;
+                if (i < c) {  // cell i lies between the vertex planes i and i+1
+                    const int cmin = E - max(__ldg(lo + i), __ldg(lo + i + 1)), cmax = max(__ldg(hi + i), __ldg(hi + i + 1));
+                    reach = (cmax >= clo) && (cmin <= chi);
+                }
+                const unsigned bal = __ballot_sync(0xFFFFFFFFu, reach);
+                if (bal) {
+                    first = min(first, i0 + __ffs(bal) - 1);
+                    last = max(last, i0 + 31 - __clz(bal));
+                }
+            }
+            if (lane == 0) { s_rng[2 * warp] = first; s_rng[2 * warp + 1] = last; }
+        }
+        if (tid == 0) s_pairs = 0;
+        __syncthreads();
+        ci0 = s_rng[0]; cj0 = s_rng[2]; ck0 = s_rng[4];
+        const int ni = max(s_rng[1] - ci0 + 1, 0);
+        nj = max(s_rng[3] - cj0 + 1, 0);
+        nk = max(s_rng[5] - ck0 + 1, 0);
+        ncell = (u32)ni * (u32)nj * (u32)nk;
+        small_box = ncell < (1u << 21);
+        rnk = 1.0f / (float)max(nk, 1);
+        rnj = 1.0f / (float)max(nj, 1);
+        if (SPARSE && ncell == 0) {
+            if (tid == 0) so.table[b] = TILE_EMPTY;
+            return;
+        }
     }
     for (int i = tid; i < img_words; i += NT) img[i] = 0;
-    if (tid < 33) s_magic[tid] = tid ? (65535 + tid) / tid : 0;
     if (tid == 0) s_large = 0;
     u32 seen_large = 0;
-    for (u32 base = beg; base < end; base += NT) {
-        __syncthreads();
-        const int n = min((u32)NT, end - base);
-        int nr = 0;
-        if (tid < n) {
+    for (;;) {
+        int n, nr = 0;
+        if (!LATTICE) {
+            if (base >= end) break;
+            __syncthreads();
+            n = min((u32)NT, end - base);
+            if (tid < n) {
+                int* r = rec + rec_off(tid);
+                const u32 t = list[base + tid];
+                const int4 id = p.lcx ? lattice_ids(p, t) : __ldg(p.tets + t);
+                if (p.pow2) setup_pair<true, false>(p, g, id, r);
+                else setup_pair<false, false>(p, g, id, r);
+                if (r[6] == 0) atomicAdd(&s_large, 1u);
+                nr = r[3];  // >= 1 for every pair: large pairs carry a one-row header that draws nothing
+            }
+            base += NT;
+        } else {
+            // fill this warp's queue until it holds a batch's worth.  A chunk is 32 cells of the index box, one per
+            // lane: decode the cell, fetch its keep byte (a chunk without kept tets costs just that).  Its candidates
+            // are then taken in groups of 5 cells x 6 tets (lane = (lane_c, lane_q), the cell's data by shuffle): a lane
+            // whose keep bit is set gathers its tet and takes the exact local box; the tets that reach the tile are
+            // appended to the queue.  When the queue is full in mid-chunk the walk stops after group grp and the next
+            // batch resumes there (the chunk's decode is simply done again).
+            u32* wq = s_wq[warp];
+            while (wq_n < 32 && chunk * 32u < ncell) {
+                const u32 cell = chunk * 32u + lane;
+                u32 kb = 0;
+                int v0 = 0;
+                if (cell < ncell) {
+                    u32 t2, di;
+                    if (small_box) {  // exact for cell < 2^21: (cell + 0.5)/nk is at least 0.5/nk away from an integer
+                        t2 = (u32)__float2int_rz(((float)cell + 0.5f) * rnk);
+                        di = (u32)__float2int_rz(((float)t2 + 0.5f) * rnj);
+                    } else {
+                        t2 = cell / (u32)nk;
+                        di = t2 / (u32)nj;
+                    }
+                    const u32 i = ci0 + di, j = cj0 + (t2 - di * (u32)nj), k = ck0 + (cell - t2 * (u32)nk);
+                    kb = __ldg(p.keep + (size_t)(((cell_base + i) * p.lcy + j) * p.lcz + k)) & 63u;
+                    v0 = (int)(((vert_base + i) * (p.lcy + 1) + j) * (p.lcz + 1) + k);
+                }
+                const unsigned any = __ballot_sync(0xFFFFFFFFu, kb != 0);
+                if (any) {
+                    for (; grp < 7; ++grp) {
+                        if (((any >> (5 * grp)) & 31u) == 0) continue;  // none of the group's five cells keeps a tet
+                        const int src = 5 * grp + lane_c;
+                        const u32 kbs = __shfl_sync(0xFFFFFFFFu, kb, src & 31);
+                        const int v0s = __shfl_sync(0xFFFFFFFFu, v0, src & 31);
+                        bool hit = false;
+                        if (lane < 30 && src < 32 && ((kbs >> lane_q) & 1u)) {
+                            const Tet q = gather_tet<true>(p, make_int4(v0s, v0s + lane_a1, v0s + lane_a12, v0s + a123));
+                            LocalBox B;
+                            hit = p.pow2 ? local_box<true>(p, g, q, B) : local_box<false>(p, g, q, B);
+                        }
+                        const unsigned bal = __ballot_sync(0xFFFFFFFFu, hit);
+                        if (hit) wq[wq_n + __popc(bal & ((1u << lane) - 1u))] = ((u32)v0s << 3) | (u32)lane_q;
+                        wq_n += __popc(bal);
+                        if (wq_n >= 32) { ++grp; break; }
+                    }
+                } else {
+                    grp = 7;
+                }
+                if (grp >= 7) { grp = 0; chunk += NW; }
+            }
+            __syncwarp();
+            const int take = min(32, wq_n);
+            if (!__syncthreads_or(take > 0)) break;  // (also the barrier that frees rec and s_incl)
+            n = NT;
             int* r = rec + rec_off(tid);
-            const u32 t = list[base + tid];
-            const int4 id = p.lcx ? lattice_ids(p, t) : __ldg(p.tets + t);
-            if (p.pow2) setup_pair<true>(p, g, id, s_magic, r);
-            else setup_pair<false>(p, g, id, s_magic, r);
-            if (r[6] == 0) atomicAdd(&s_large, 1u);
-            nr = r[3];  // >= 1 for every pair: large pairs carry a one-row header that draws nothing
+            bool drawn = false;
+            u32 carry = 0;
+            if (lane + 32 < wq_n) carry = wq[lane + 32];
+            if (lane < take) {
+                const u32 e = wq[lane];
+                const int v0 = (int)(e >> 3), q = (int)(e & 7u);
+                const int a1 = (q < 2) ? lat_sx : (q < 4) ? lat_sy : 1;
+                const int a3 = (q == 3 || q == 5) ? lat_sx : (q == 1 || q == 4) ? lat_sy : 1;
+                const int4 id = make_int4(v0, v0 + a1, v0 + a123 - a3, v0 + a123);
+                drawn = p.pow2 ? setup_pair<true, true>(p, g, id, r) : setup_pair<false, true>(p, g, id, r);
+                if (r[6] == 0) atomicAdd(&s_large, 1u);
+            } else {
+                null_record(r, g.img_saddr);
+            }
+            nr = r[3];
+            my_pairs += __popc(__ballot_sync(0xFFFFFFFFu, drawn));
+            __syncwarp();
+            if (lane + 32 < wq_n) wq[lane] = carry;  // the rest of the queue moves to the front
+            wq_n -= take;
         }
         int incl = nr;
 #pragma unroll
@@ -1045,13 +1281,14 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(const __grid_constant__ Para
             int pi = w * 32 + j;
             int rr = local - (j ? inc[j - 1] : 0);
             LaneRec L;
-            lane_load(rec + rec_off(pi), L);
+            u32 ra = rec_saddr + 4u * (u32)rec_off(pi);
+            lane_load(ra, L);
             for (;;) {
                 lane_row(L, rr, img_stride);
                 if (--cnt == 0) break;
                 if (++rr == L.A.w) {  // next pair (every pair has at least one row)
-                    ++pi;
-                    lane_load(rec + rec_off(pi), L);
+                    ra += ((++pi & 3) == 0) ? 4u * SREC_W + 16u : 4u * SREC_W;  // rec_off: 16-byte pad after every 4th record
+                    lane_load(ra, L);
                     rr = 0;
                 }
             }
@@ -1066,8 +1303,14 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(const __grid_constant__ Para
             }
         }
     }
+    if (LATTICE && lane == 0 && my_pairs) atomicAdd(&s_pairs, my_pairs);
     __syncthreads();
     if (tid == 0 && s_large) atomicAdd(hdr + H_LARGE, s_large);
+    if (LATTICE && tid == 0 && s_pairs) {  // the statistics K2 leaves in the header on the binned path
+        const u32 np = s_pairs, old = atomicAdd(hdr + H_TOTAL, np);
+        if (old + np < old) atomicAdd(hdr + H_TOTAL_HI, 1u);
+        atomicAdd(hdr + H_NONEMPTY, 1u);
+    }
     tile_epilogue<NT, SPARSE>(p, img, img_stride, b, bx, m, g.Y0, g.Z0, bits, hdr, so, tid);
 }
 
@@ -1258,7 +1501,9 @@ extern "C" int vox_set_tile(vox_ctx* ctx, int ty, int tz) {
 }
 
 extern "C" int vox_set_variant(vox_ctx* ctx, int variant) {
-    if (!ctx || variant != 0) return VOX_EINVAL;  // no A/B variant is compiled in at present
+    // 0: default.  1: lattice input goes through the binning passes K1-K3 like a tet array (cross-check of the
+    // fused lattice path; no effect on explicit tets)
+    if (!ctx || (variant != 0 && variant != 1)) return VOX_EINVAL;
     ctx->variant = variant;
     return VOX_OK;
 }
@@ -1295,10 +1540,19 @@ extern "C" int vox_lattice(vox_ctx* ctx, const int32_t* d_verts, int cx, int cy,
     p.lcx = cx; p.lcy = cy; p.lcz = cz;
     p.V = V;
     p.T = 6 * cells;
-    if (!ctx->tile_user) auto_tile(p, p.T);
+    // (T counts the absent tets too: a carved lattice keeps a fraction, a third is assumed for the tile choice; larger
+    //  tiles also mean a thinner rim of candidate cells per tile on the fused path)
+    if (!ctx->tile_user) auto_tile(p, p.T / 3);
     ctx->have_tets = true;
     ctx->pairs_planned = -1;
     return VOX_OK;
+}
+
+// lattice input takes the fused path (K0 + K4, no binning) unless variant 1 asks for the binned one or the lattice
+// is beyond what k0_slabs / the candidate queue were sized for
+static bool lattice_fused(const vox_ctx* ctx) {
+    const Params& p = ctx->p;
+    return p.lcx > 0 && ctx->variant == 0 && p.lcx <= 4096 && p.lcy <= 4096 && p.lcz <= 4096 && p.V < (1ll << 28);
 }
 
 extern "C" size_t vox_grid_words(const vox_ctx* ctx) {
@@ -1315,6 +1569,8 @@ extern "C" size_t vox_workspace_fixed_bytes(const vox_ctx* ctx) {
 extern "C" size_t vox_workspace_bytes(const vox_ctx* ctx) {
     if (!ctx) return 0;
     const Params& p = ctx->p;
+    if (lattice_fused(ctx))  // header + slabs + the packed vertex copy: no counters, no range array, no pair list
+        return ws_layout(p).counts + align256((size_t)p.V * 16);
     i64 pairs = ctx->pairs_planned >= 0 ? ctx->pairs_planned : 4 * p.T + (i64)p.NB;
     if (pairs < 1) pairs = 1;
     return ws_layout(p).fixed_end + align256((size_t)pairs * 4);
@@ -1406,12 +1662,42 @@ static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t w
     if (!ctx->have_tets) return VOX_ESTATE;
     Params& p = ctx->p;
     WsLayout L = ws_layout(p);
-    if (ws_bytes < L.fixed_end + 4) return VOX_EWORKSPACE;
-    size_t cap = (ws_bytes - L.list) / 4;
-    p.cap = (u32)(cap > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : cap);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char* ws = (char*)d_workspace;
     cudaEvent_t* ev = ctx->tm_ev ? ctx->tm_ev + (size_t)(ctx->tm_next % ctx->tm_slots) * TM_EV : NULL;
+    if (lattice_fused(ctx)) {  // K0 (vertex-plane slabs) + K4 enumerating its own candidates
+        if (ws_bytes < L.counts + (size_t)p.V * 16) return VOX_EWORKSPACE;
+        u32* hdr = (u32*)(ws + L.hdr);
+        int* slab = (int*)(ws + L.slab);
+        p.verts4 = (const int4*)(ws + L.counts);  // (the binned path's arrays are not used: their room holds the copy)
+        if (ev) CK(cudaEventRecord(ev[0], st));
+        CK(cudaMemsetAsync(ws + L.hdr, 0, L.counts - L.hdr, st));
+        // enough CTAs for two waves: one per (x plane, chunk of y rows, mesh)
+        const i64 planes = (i64)(p.lcx + 1) * p.batch;
+        int chunks = (int)((2 * 148 * 4 + planes - 1) / planes);
+        if (chunks > p.lcy + 1) chunks = p.lcy + 1;
+        if (chunks > 65535) chunks = 65535;
+        const int jchunk = (p.lcy + 1 + chunks - 1) / chunks;
+        dim3 grid0((unsigned)(p.lcx + 1), (unsigned)((p.lcy + 1 + jchunk - 1) / jchunk), (unsigned)p.batch);
+        k0_slabs<<<grid0, 256, 2 * (size_t)(p.lcz + 1) * 4, st>>>(p.verts, p.lcx, p.lcy, p.lcz, p.ex, p.ey, p.ez, jchunk, slab,
+                                                                  (int4*)(ws + L.counts));
+        count_launch();
+        if (ev) { CK(cudaEventRecord(ev[1], st)); CK(cudaEventRecord(ev[2], st)); CK(cudaEventRecord(ev[3], st)); }
+        const SparseOut so = ctx->sparse;
+        if (so.table) k4_flat<128, 8, true, true><<<p.NB, 128, 0, st>>>(p, NULL, NULL, d_bits_out, hdr, so, slab);
+        else k4_flat<128, 8, false, true><<<p.NB, 128, 0, st>>>(p, NULL, NULL, d_bits_out, hdr, so, slab);
+        count_launch();
+        CK(cudaGetLastError());
+        if (ev) {
+            CK(cudaEventRecord(ev[4], st));
+            ctx->tm_next++;
+        }
+        return VOX_OK;
+    }
+    p.verts4 = NULL;
+    if (ws_bytes < L.fixed_end + 4) return VOX_EWORKSPACE;
+    size_t cap = (ws_bytes - L.list) / 4;
+    p.cap = (u32)(cap > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : cap);
     int rc = enqueue_count_scan(ctx, st, ws, ev, true);
     if (rc) return rc;
     u32* hdr = (u32*)(ws + L.hdr);
@@ -1427,10 +1713,10 @@ static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t w
     if (ev) CK(cudaEventRecord(ev[3], st));
     const SparseOut so = ctx->sparse;
     if (so.table) {
-        k4_flat<128, 8, true><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);
+        k4_flat<128, 8, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so, NULL);
         count_launch();
     } else {
-        k4_flat<128, 8, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so);  // 64 regs, 32 warps/SM
+        k4_flat<128, 8, false, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so, NULL);  // 64 regs, 32 warps/SM
         count_launch();
     }
     CK(cudaGetLastError());

@@ -84,8 +84,9 @@ def test_misaligned_workspace_variant_and_tile_count_limits(lib):
     assert lib.vox_run(c, None, ctypes.c_void_p(256 + 4), 1 << 20, ctypes.c_void_p(256)) == -1
     assert lib.vox_plan(c, None, ctypes.c_void_p(256 + 8), 1 << 20, None) == -1
     assert lib.vox_validate(c, None, ctypes.c_void_p(256 + 4), 1 << 20) == -1
-    # no A/B variant is compiled in: refused, not ignored
+    # variants: 0 default, 1 binned lattice path; anything else is refused, not ignored
     assert lib.vox_set_variant(c, 0) == 0
+    assert lib.vox_set_variant(c, 1) == 0
     assert lib.vox_set_variant(c, 3) == -1
     lib.vox_destroy(c)
     # one CTA per tile: more than 2^31 - 1 tiles cannot be launched -> VOX_ERANGE at create / set_tile

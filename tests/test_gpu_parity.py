@@ -96,14 +96,14 @@ def test_parity_is_tile_independent(name, tile):
 
 
 def test_unknown_kernel_variant_is_refused():
-    # no A/B variant is compiled in: a non-zero variant must be refused, never silently ignored (dense or sparse)
+    # variants 0 (default) and 1 (binned lattice path) exist; any other must be refused, never silently ignored
     import paper_2106_01326_b200 as pkg
 
     with pytest.raises(pkg.VoxError) as ei:
         pkg.Voxelizer((32, 32, 32), variant=3)
     assert ei.value.code == -1
     with pytest.raises(pkg.VoxError):
-        pkg.Pipe((32, 32, 32), depth=1, max_V=4, max_T=1, variant=1)
+        pkg.Pipe((32, 32, 32), depth=1, max_V=4, max_T=1, variant=2)
 
 
 def test_estimated_workspace_path():

@@ -39,8 +39,12 @@ def _cases():
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("variant", [0, 1], ids=["fused", "binned"])
 @pytest.mark.parametrize("idx", range(5))
-def test_gpu_lattice_input_matches_oracle(idx):
+def test_gpu_lattice_input_matches_oracle(idx, variant):
+    """variant 0: the fused lattice path (K0 slabs + tiles enumerating their own candidate cells, no K1-K3);
+    variant 1: the same input through the binning passes.  Both must give the oracle's grid and count the same
+    (tet, tile) pairs as the tet array written out."""
     import torch
 
     import paper_2106_01326_b200 as pkg
@@ -48,16 +52,26 @@ def test_gpu_lattice_input_matches_oracle(idx):
     name, m, cells = _cases()[idx]
     exp = oracle.voxelize(m.verts, m.tets, m.grid, m.extent, tet_offsets=m.tet_offsets)
     keep = meshgen.lattice_form(m, cells)
-    vz = pkg.Voxelizer(m.grid, m.extent, m.batch)
+    vz = pkg.Voxelizer(m.grid, m.extent, m.batch, variant=variant)
     vz.set_lattice(torch.from_numpy(m.verts).cuda(), cells, torch.from_numpy(keep).cuda())
+    if variant == 0:    # header + slabs + the 16-byte vertex copy: no counters, no range array, no pair list
+        assert vz.workspace_bytes <= 1024 + 8 * m.batch * (sum(cells) + 3) + 16 * m.V + 768
     pairs = vz.plan()
     got = vz.run().cpu().numpy().view(np.uint32)
     st = vz.status()
+    # sparse output through the same path
+    from oracle import sparse
+    ts = vz.tile_shape
+    nb = m.batch * ts["nbx"] * ts["nby"] * ts["nbz"]
+    tab, pay = vz.run_sparse(nb)
+    mixed = vz.sparse_status()["mixed_tiles"]
     vz.close()
     assert np.array_equal(got, exp), f"{name}: {(got != exp).sum()} words differ"
+    assert sparse.check_table(tab.cpu().numpy(), pay.cpu().numpy(), exp, ts["ty"], ts["tz"]) == mixed
     # the same pairs as with the tets written out
     ref = pkg.voxelize(m.verts, m.tets, m.grid, m.extent, tet_offsets=m.tet_offsets if m.batch > 1 else None)
     assert np.array_equal(ref, exp) and pkg.voxelize.last_status["pairs"] == st["pairs"] == pairs
+    assert pkg.voxelize.last_status["large_pairs"] == st["large_pairs"]
 
 
 @pytest.mark.gpu
