@@ -413,6 +413,9 @@ __global__ void __launch_bounds__(256) k3_scatter(Params p, const uint2* __restr
             m = mesh_of(p, t);
         }
     }
+    // (tried, round 2: one atomic per (tet, tile) with up to 8 in flight per thread instead of the lockstep aggregation --
+    //  2-3.5x slower, 0.15 against 0.072 ms on cfg4, 0.32 against 0.092 on the 10^7-tet mesh: the cursors of a tile are hot
+    //  addresses and the number of atomics, not their latency, is what binds)
     // warp-aggregated cursor bump (same stepping as K1): one atomic per distinct tile per step,
     // the lanes of a group take consecutive slots (order inside a tile list is irrelevant: OR)
     const int lane = threadIdx.x & 31;
@@ -1415,7 +1418,10 @@ static void set_tile(Params& p, int ty, int tz) {
 static void auto_tile(Params& p, i64 T) {
     int ty = 32, tz = 32;
     auto tiles = [&](int a, int b) { return (i64)p.batch * (p.nx / 32) * ((p.ny + a - 1) / a) * ((p.nz + b - 1) / b); };
-    while ((tiles(ty, tz) < 4 * 1184 || T / tiles(ty, tz) > 1024) && (ty > 8 || tz > 8)) {
+    // (third clause, round 2: below ~16 waves the last wave's idle SMs show -- cfg3 ran 27% of K4 with SMs idle on
+    //  8192 tiles of 32x16x16 and is 17% faster on 32768 of 32x8x8 -- so keep halving while a tile still has work)
+    while ((tiles(ty, tz) < 4 * 1184 || T / tiles(ty, tz) > 1024 || (tiles(ty, tz) < 16 * 1184 && T / tiles(ty, tz) > 128)) &&
+           (ty > 8 || tz > 8)) {
         if (tz >= ty && tz > 8) tz >>= 1; else ty >>= 1;
     }
     while (ty < 32 && (p.ny + ty - 1) / ty > 1024) ty <<= 1;
