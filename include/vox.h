@@ -259,6 +259,13 @@ int vox_probe_int32(void* cuda_stream, int kind, int blocks, int iters, uint32_t
  * copies are not kernels).  bench.py reports the difference across its timed region as `gpu_launches`. */
 uint64_t vox_kernel_launches(void);
 
+/* Checked build (libvox_checked.so, compiled with -DVOX_CHECKS by paper_2106_01326_b200.build.build_checked): every
+ * index the kernels form (tile ids, list entries, vertex ids, record slots, image-row addresses, queue slots, grid
+ * words) is tested before use and the code of the first violated check is kept on the device.  SYNCHRONISES the
+ * device, returns 1 and stores that code (0 = none) in *code_out, then clears it; the normal library compiles no
+ * check and returns 0.  Test instrumentation: compute-sanitizer is closed on this pool (profiles/r02_sanitizers.md). */
+int vox_debug_check_status(uint32_t* code_out);
+
 const char* vox_strerror(int code);
 const char* vox_last_error(const vox_ctx* ctx); /* CUDA error text of the last VOX_ECUDA */
 

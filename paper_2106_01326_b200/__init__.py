@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     Pipe,
     VoxError,
     Voxelizer,
+    debug_check_status,
     kernel_launches,
     lib_path,
     load_library,

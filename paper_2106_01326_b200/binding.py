@@ -5,7 +5,8 @@ import ctypes
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libvox.so")
+# VOX_LIB selects another build of the same library (tests: the checked build libvox_checked.so)
+_LIB_PATH = os.environ.get("VOX_LIB") or os.path.join(_HERE, "libvox.so")
 _lib = None
 
 # every symbol include/vox.h declares
@@ -18,6 +19,7 @@ EXPORTS = [
     "vox_pipe_bind", "vox_pipe_submit", "vox_pipe_wait", "vox_pipe_last_error",
     "vox_tile_shape", "vox_run_sparse", "vox_sparse_status", "vox_pipe_submit_sparse", "vox_pipe_tile_shape",
     "vox_pipe_reserve_pairs", "vox_occupancy", "vox_lattice", "vox_pipe_submit_lattice", "vox_kernel_launches",
+    "vox_debug_check_status",
 ]
 
 
@@ -82,6 +84,7 @@ def load_library():
         "vox_lattice": (i32, [vp, vp, i32, i32, i32, vp]),
         "vox_pipe_submit_lattice": (i32, [vp, vp, i32, i32, i32, vp, vp, vp, i64, ctypes.POINTER(i64)]),
         "vox_kernel_launches": (ctypes.c_uint64, []),
+        "vox_debug_check_status": (i32, [ctypes.POINTER(ctypes.c_uint32)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -502,6 +505,15 @@ def voxelize_host(verts, tets, grid, extent=(65536, 65536, 65536), tet_offsets=N
         return out.numpy().view(np.uint32)
     finally:
         vz.close()
+
+
+def debug_check_status():
+    """vox_debug_check_status: (checks_compiled_in, code of the first violated check or 0).  Synchronises the device."""
+    code = ctypes.c_uint32(0)
+    rc = load_library().vox_debug_check_status(ctypes.byref(code))
+    if rc < 0:
+        raise VoxError(rc, "vox_debug_check_status")
+    return bool(rc), int(code.value)
 
 
 def kernel_launches() -> int:

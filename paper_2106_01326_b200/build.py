@@ -20,6 +20,21 @@ NVCC_FLAGS = [
 ]
 
 
+LIB_CHECKED = os.path.join(_HERE, "libvox_checked.so")
+
+
+def build_checked(force: bool = False) -> str:
+    """The same source with -DVOX_CHECKS: device-side bounds checks on every index the kernels form
+    (vox_debug_check_status; tests/test_gpu_checked_build.py)."""
+    if force or not os.path.exists(LIB_CHECKED) or any(
+            os.path.getmtime(f) > os.path.getmtime(LIB_CHECKED) for f in (SRC, HDR)):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        tmp = LIB_CHECKED + f".tmp{os.getpid()}"
+        subprocess.check_call([nvcc] + NVCC_FLAGS + ["-DVOX_CHECKS", "-o", tmp, SRC])
+        os.replace(tmp, LIB_CHECKED)
+    return LIB_CHECKED
+
+
 def needs_build() -> bool:
     if not os.path.exists(LIB):
         return True

@@ -86,6 +86,26 @@ enum { BIG_TILES = 64, BIG_CAP = 4096, RANGE_BIG = 0x40000000 };
 
 static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
+// Checked build (-DVOX_CHECKS, libvox_checked.so): every index the kernels form is tested before it is used and the
+// first violated check's code is kept in g_check (vox_debug_check_status).  compute-sanitizer is closed on this
+// pool (profiles/r02_sanitizers.md): these bounds checks, run under the parity suite's small cases, stand in for
+// memcheck; the barrier structure that stands in for racecheck is written out there as well.  The normal build
+// compiles none of it.
+#ifdef VOX_CHECKS
+__device__ unsigned int g_check = 0;
+#define VOX_CHECK(cond, code)                         \
+    do {                                              \
+        if (!(cond)) atomicCAS(&g_check, 0u, (unsigned)(code)); \
+    } while (0)
+#else
+#define VOX_CHECK(cond, code) do { } while (0)
+#endif
+enum {  // check codes
+    CK_K1_TILE = 101, CK_K1_VERT = 102, CK_K2_TILE = 201, CK_K3_TILE = 301, CK_K3_RANGE = 302,
+    CK_K4_LIST = 401, CK_K4_VERT = 402, CK_K4_BOX = 403, CK_K4_ROWADDR = 404, CK_K4_RECIDX = 405, CK_K4_QUEUE = 406,
+    CK_K4_CELL = 407, CK_K4_ROWS = 408, CK_K4_STORE = 409, CK_K4_LARGEBOX = 410, CK_K0_VERT = 501
+};
+
 // kernels launched by this library in this process (vox_kernel_launches: bench.py's gpu_launches)
 static unsigned long long g_launches = 0;
 static inline void count_launch() { __atomic_fetch_add(&g_launches, 1ull, __ATOMIC_RELAXED); }
@@ -162,6 +182,7 @@ __device__ __forceinline__ int4 lattice_ids(const Params& p, i64 t) {
 
 __device__ __forceinline__ Tet load_tet(const Params& p, i64 t) {
     const int4 id = p.lcx ? lattice_ids(p, t) : __ldg(p.tets + t);
+    VOX_CHECK(id.x >= 0 && id.x < p.V && id.y >= 0 && id.y < p.V && id.z >= 0 && id.z < p.V && id.w >= 0 && id.w < p.V, CK_K1_VERT);
     const int32_t* v = p.verts;
     Tet q;
     q.ax = __ldg(v + 3 * (i64)id.x); q.ay = __ldg(v + 3 * (i64)id.x + 1); q.az = __ldg(v + 3 * (i64)id.x + 2);
@@ -251,6 +272,7 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
         if (!act) break;
         if (live) {
             const u32 b = ((((u32)m * p.nbz + cz) * p.nby + cy) * p.nbx) + cx;
+            VOX_CHECK(b < p.NB, CK_K1_TILE);
             const unsigned peers = __match_any_sync(act, b);
             if (lane == __ffs(peers) - 1) atomicAdd(counts + b, (u32)__popc(peers));
             if (++cx > b1x) {
@@ -293,7 +315,10 @@ __global__ void __launch_bounds__(1024) k2_scan(Params p, const uint2* __restric
         const uint2 r = range[t];
         const int m = mesh_of(p, t);
         const u32 n = range_tiles(r);
-        for (u32 idx = threadIdx.x; idx < n; idx += 1024u) atomicAdd(counts + range_tile(p, r, m, idx), 1u);
+        for (u32 idx = threadIdx.x; idx < n; idx += 1024u) {
+            VOX_CHECK(range_tile(p, r, m, idx) < p.NB, CK_K2_TILE);
+            atomicAdd(counts + range_tile(p, r, m, idx), 1u);
+        }
     }
     if (nbig) {
         __threadfence();
@@ -424,6 +449,7 @@ __global__ void __launch_bounds__(256) k3_scatter(Params p, const uint2* __restr
         if (!act) break;
         if (live) {
             const u32 b = ((((u32)m * p.nbz + cz) * p.nby + cy) * p.nbx) + cx;
+            VOX_CHECK(b < p.NB, CK_K3_TILE);
             const unsigned peers = __match_any_sync(act, b);
             const int leader = __ffs(peers) - 1;
             u32 base = 0;
@@ -625,6 +651,7 @@ __device__ __noinline__ void raster_large_rec(const int* rec, u32* img, int lane
     const u32 box = (u32)rec[5];
     const int x0 = box & 31, x1 = (box >> 5) & 31, y0 = (box >> 10) & 31, y1 = (box >> 15) & 31;
     const int z0 = (box >> 20) & 31, z1 = (box >> 25) & 31;
+    VOX_CHECK(x0 <= x1 && y0 <= y1 && z0 <= z1 && (z1 * img_stride + y1) < 32 * (32 + IMG_SKEW), CK_K4_LARGEBOX);
     bool all_in = true, any_out = false;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
@@ -796,6 +823,7 @@ __device__ __forceinline__ void centre_range(int lo, int hi, int h, int sh, int&
 // the four vertices of a tet: one 16-byte load each from K0's packed copy (fused lattice path), else 3 x 4 bytes
 template <bool V4>
 __device__ __forceinline__ Tet gather_tet(const Params& p, int4 id) {
+    VOX_CHECK(id.x >= 0 && id.x < p.V && id.y >= 0 && id.y < p.V && id.z >= 0 && id.z < p.V && id.w >= 0 && id.w < p.V, CK_K4_VERT);
     Tet q;
     if (V4) {
         const int4 a = __ldg(p.verts4 + id.x), b = __ldg(p.verts4 + id.y), c = __ldg(p.verts4 + id.z), d = __ldg(p.verts4 + id.w);
@@ -837,6 +865,7 @@ __device__ __forceinline__ bool setup_pair(const Params& p, const TileGeo& g, in
     LocalBox B;
     const bool hit = local_box<POW2>(p, g, q, B);
     const int x0 = B.x0, x1 = B.x1, y0 = B.y0, y1 = B.y1, z0 = B.z0, z1 = B.z1;
+    VOX_CHECK(!hit || (x0 >= 0 && x1 <= 31 && y0 >= 0 && y1 <= g.ymax && z0 >= 0 && z1 <= g.zmax && g.ymax <= 31 && g.zmax <= 31), CK_K4_BOX);
     if (!hit) {
         null_record(rec, g.img_saddr);
         return false;
@@ -930,7 +959,7 @@ __device__ __forceinline__ void lane_load(u32 rec_saddr, LaneRec& L) {
 }
 
 // one row rr of the pair held in L: the four exact bounds, the span, one OR into the tile image
-__device__ __forceinline__ void lane_row(const LaneRec& L, int rr, int img_stride) {
+__device__ __forceinline__ void lane_row(const LaneRec& L, int rr, int img_stride, u32 img_lo, u32 img_hi) {
     const int zz = (int)(((u32)rr * (u32)L.B.y) >> 16);
     const int yy = rr - zz * L.A.z;
     const int b0 = span_bound(L.P0.w + L.P0.y * yy + L.P0.z * zz, L.P0.x, L.IV.x);
@@ -945,6 +974,8 @@ __device__ __forceinline__ void lane_row(const LaneRec& L, int rr, int img_strid
     const int upper = min(min(L.A.y, b3), min(u1, u2));
     const int n = upper - lower;
     const u32 saddr = (u32)L.B.x + 4u * (u32)(zz * img_stride + yy);
+    VOX_CHECK(rr >= 0 && rr < L.A.w && yy >= 0 && yy < L.A.z && zz >= 0 && zz <= 31, CK_K4_ROWS);
+    VOX_CHECK(saddr >= img_lo && saddr < img_hi && (saddr & 3u) == 0, CK_K4_ROWADDR);
     // branch-free: PTX shifts clamp at 32, so n <= 0 gives word 0 and the OR is a no-op
     asm volatile(
         "{\n\t.reg .b32 m, s;\n\t"
@@ -967,8 +998,10 @@ __device__ __forceinline__ void tile_epilogue(const Params& p, const u32* img, i
         for (int i = tid; i < rows; i += NT) {
             const int z = i >> p.ty_log, y = i & (TY - 1);
             const int gy = Y0 + y, gz = Z0 + z;
-            if (gy < p.ny && gz < p.nz)
+            if (gy < p.ny && gz < p.nz) {
+                VOX_CHECK((((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx < (size_t)p.batch * p.nz * p.ny * p.wpr, CK_K4_STORE);
                 bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[z * img_stride + y];
+            }
         }
         return;
     }
@@ -1038,6 +1071,7 @@ __global__ void __launch_bounds__(256) k0_slabs(const int32_t* __restrict__ vert
         const int32_t* row = verts + 3 * v0;
         for (int k = lane; k <= cz; k += 32) {
             const int x = __ldg(row + 3 * k), y = __ldg(row + 3 * k + 1), z = __ldg(row + 3 * k + 2);
+            VOX_CHECK(v0 + k < (size_t)gridDim.z * (cx + 1) * (cy + 1) * (cz + 1), CK_K0_VERT);
             verts4[v0 + k] = make_int4(x, y, z, 0);
             mxhi = max(mxhi, x); mxlo = max(mxlo, ex - x);
             myhi = max(myhi, y); mylo = max(mylo, ey - y);
@@ -1172,6 +1206,7 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(const __grid_constant__ Para
             if (tid < n) {
                 int* r = rec + rec_off(tid);
                 const u32 t = list[base + tid];
+                VOX_CHECK((i64)t < p.T && base + tid < p.cap, CK_K4_LIST);
                 const int4 id = p.lcx ? lattice_ids(p, t) : __ldg(p.tets + t);
                 if (p.pow2) setup_pair<true, false>(p, g, id, r);
                 else setup_pair<false, false>(p, g, id, r);
@@ -1201,6 +1236,7 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(const __grid_constant__ Para
                         di = t2 / (u32)nj;
                     }
                     const u32 i = ci0 + di, j = cj0 + (t2 - di * (u32)nj), k = ck0 + (cell - t2 * (u32)nk);
+                    VOX_CHECK(i < (u32)p.lcx && j < (u32)p.lcy && k < (u32)p.lcz, CK_K4_CELL);
                     kb = __ldg(p.keep + (size_t)(((cell_base + i) * p.lcy + j) * p.lcz + k)) & 63u;
                     v0 = (int)(((vert_base + i) * (p.lcy + 1) + j) * (p.lcz + 1) + k);
                 }
@@ -1218,6 +1254,7 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(const __grid_constant__ Para
                             hit = p.pow2 ? local_box<true>(p, g, q, B) : local_box<false>(p, g, q, B);
                         }
                         const unsigned bal = __ballot_sync(0xFFFFFFFFu, hit);
+                        VOX_CHECK(wq_n + __popc(bal) <= 64, CK_K4_QUEUE);
                         if (hit) wq[wq_n + __popc(bal & ((1u << lane) - 1u))] = ((u32)v0s << 3) | (u32)lane_q;
                         wq_n += __popc(bal);
                         if (wq_n >= 32) { ++grp; break; }
@@ -1283,14 +1320,16 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(const __grid_constant__ Para
                 if (inc[j + step - 1] <= local) j += step;
             int pi = w * 32 + j;
             int rr = local - (j ? inc[j - 1] : 0);
+            VOX_CHECK(pi >= 0 && pi < NT && rr >= 0, CK_K4_RECIDX);
             LaneRec L;
             u32 ra = rec_saddr + 4u * (u32)rec_off(pi);
             lane_load(ra, L);
             for (;;) {
-                lane_row(L, rr, img_stride);
+                lane_row(L, rr, img_stride, g.img_saddr, g.img_saddr + 4u * (u32)img_words);
                 if (--cnt == 0) break;
                 if (++rr == L.A.w) {  // next pair (every pair has at least one row)
                     ra += ((++pi & 3) == 0) ? 4u * SREC_W + 16u : 4u * SREC_W;  // rec_off: 16-byte pad after every 4th record
+                    VOX_CHECK(pi < NT && ra == rec_saddr + 4u * (u32)rec_off(pi), CK_K4_RECIDX);
                     lane_load(ra, L);
                     rr = 0;
                 }
@@ -2186,6 +2225,20 @@ extern "C" int vox_probe_int32(void* cuda_stream, int kind, int blocks, int iter
 }
 
 extern "C" uint64_t vox_kernel_launches(void) { return __atomic_load_n(&g_launches, __ATOMIC_RELAXED); }
+
+extern "C" int vox_debug_check_status(uint32_t* code_out) {
+#ifdef VOX_CHECKS
+    unsigned int c = 0, zero = 0;
+    if (cudaDeviceSynchronize() != cudaSuccess) return VOX_ECUDA;
+    if (cudaMemcpyFromSymbol(&c, g_check, sizeof(c)) != cudaSuccess) return VOX_ECUDA;
+    if (cudaMemcpyToSymbol(g_check, &zero, sizeof(zero)) != cudaSuccess) return VOX_ECUDA;
+    if (code_out) *code_out = c;
+    return 1;
+#else
+    if (code_out) *code_out = 0;
+    return 0;
+#endif
+}
 
 extern "C" const char* vox_strerror(int code) {
     switch (code) {
