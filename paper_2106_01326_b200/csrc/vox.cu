@@ -43,6 +43,7 @@ struct Params {
     int sx, sy, sz;      // h / g
     int c4x, c4y, c4z;   // -4 * (h / g): sign and scale of a stored plane coefficient (setup_pair's fast path)
     int pow2;            // every 2h and g is a power of two: shifts instead of divisions
+    int grid3;           // K4 is launched as a 3-D grid (nbx, nby, nbz*batch) rather than 1-D over the tiles
     float fit_vol, fit_ax, fit_ay, fit_az;  // setup_pair's int32 fit test: 24/g, 16*sx, 16*sy, 16*sz
     int ty_log, tz_log;  // tile = 32 x (1<<ty_log) x (1<<tz_log) voxels
     int nbx, nby, nbz;   // tiles per axis
@@ -995,12 +996,14 @@ __device__ __forceinline__ void tile_epilogue(const Params& p, const u32* img, i
     const int TY = 1 << p.ty_log;
     const int rows = 1 << (p.ty_log + p.tz_log);
     if (!SPARSE) {
+        // word of row (y,z) = tile base + (z*ny + y)*wpr: the row offset fits 32 bits (z,y < 32, ny <= 32768, wpr <= 1024)
+        u32* base = bits + (((size_t)m * p.nz + Z0) * p.ny + Y0) * p.wpr + bx;
+        const int ylim = p.ny - Y0, zlim = p.nz - Z0;
         for (int i = tid; i < rows; i += NT) {
             const int z = i >> p.ty_log, y = i & (TY - 1);
-            const int gy = Y0 + y, gz = Z0 + z;
-            if (gy < p.ny && gz < p.nz) {
-                VOX_CHECK((((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx < (size_t)p.batch * p.nz * p.ny * p.wpr, CK_K4_STORE);
-                bits[(((size_t)m * p.nz + gz) * p.ny + gy) * p.wpr + bx] = img[z * img_stride + y];
+            if (y < ylim && z < zlim) {
+                VOX_CHECK((((size_t)m * p.nz + Z0 + z) * p.ny + Y0 + y) * p.wpr + bx < (size_t)p.batch * p.nz * p.ny * p.wpr, CK_K4_STORE);
+                base[(u32)(z * p.ny + y) * (u32)p.wpr] = img[z * img_stride + y];
             }
         }
         return;
@@ -1114,13 +1117,22 @@ __global__ void __launch_bounds__(NT, MINB) k4_flat(const __grid_constant__ Para
     __shared__ u32 s_pairs;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = NT / 32;
-    const u32 b = blockIdx.x;
-    const u32 bx = b % p.nbx;
-    u32 rest = b / p.nbx;
-    const u32 by = rest % p.nby;
-    rest /= p.nby;
-    const u32 bz = rest % p.nbz;
-    const u32 m = rest / p.nbz;
+    // tile (bx, by, bz) of mesh m: a 3-D grid (x, y, z*batch) when that fits gridDim (no divisions), else 1-D over tiles
+    u32 b, bx, by, bz, m;
+    if (p.grid3) {
+        bx = blockIdx.x; by = blockIdx.y;
+        m = (p.batch == 1) ? 0u : blockIdx.z / (u32)p.nbz;
+        bz = blockIdx.z - m * (u32)p.nbz;
+        b = ((m * p.nbz + bz) * p.nby + by) * p.nbx + bx;
+    } else {
+        b = blockIdx.x;
+        bx = b % p.nbx;
+        u32 rest = b / p.nbx;
+        by = rest % p.nby;
+        rest /= p.nby;
+        bz = rest % p.nbz;
+        m = rest / p.nbz;
+    }
     const int TY = 1 << p.ty_log, TZ = 1 << p.tz_log;
     TileGeo g;
     g.X0 = bx << 5; g.Y0 = by << p.ty_log; g.Z0 = bz << p.tz_log;
@@ -1702,6 +1714,13 @@ extern "C" int vox_sparse_status(vox_ctx* ctx, void* cuda_stream, const void* d_
     return (h[H_OVERFLOW] || h[H_PAYLOAD_OVERFLOW]) ? VOX_EWORKSPACE : VOX_OK;
 }
 
+// K4's grid: one CTA per tile, 3-D when the tile counts fit gridDim.y/z (sets p.grid3 for the kernel's decode)
+static dim3 k4_grid(Params& p) {
+    const i64 zb = (i64)p.nbz * p.batch;
+    p.grid3 = (p.nby <= 65535 && zb <= 65535) ? 1 : 0;
+    return p.grid3 ? dim3((unsigned)p.nbx, (unsigned)p.nby, (unsigned)zb) : dim3(p.NB);
+}
+
 static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes, uint32_t* d_bits_out) {
     if (((uintptr_t)d_workspace & 15) != 0) return VOX_EINVAL;  // uint2 / uint4 accesses of the workspace arrays
     if (!ctx->have_tets) return VOX_ESTATE;
@@ -1729,8 +1748,9 @@ static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t w
         count_launch();
         if (ev) { CK(cudaEventRecord(ev[1], st)); CK(cudaEventRecord(ev[2], st)); CK(cudaEventRecord(ev[3], st)); }
         const SparseOut so = ctx->sparse;
-        if (so.table) k4_flat<128, 8, true, true><<<p.NB, 128, 0, st>>>(p, NULL, NULL, d_bits_out, hdr, so, slab);
-        else k4_flat<128, 8, false, true><<<p.NB, 128, 0, st>>>(p, NULL, NULL, d_bits_out, hdr, so, slab);
+        const dim3 grid4 = k4_grid(p);
+        if (so.table) k4_flat<128, 8, true, true><<<grid4, 128, 0, st>>>(p, NULL, NULL, d_bits_out, hdr, so, slab);
+        else k4_flat<128, 8, false, true><<<grid4, 128, 0, st>>>(p, NULL, NULL, d_bits_out, hdr, so, slab);
         count_launch();
         CK(cudaGetLastError());
         if (ev) {
@@ -1757,11 +1777,12 @@ static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t w
     }
     if (ev) CK(cudaEventRecord(ev[3], st));
     const SparseOut so = ctx->sparse;
+    const dim3 grid4 = k4_grid(p);
     if (so.table) {
-        k4_flat<128, 8, true, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so, NULL);
+        k4_flat<128, 8, true, false><<<grid4, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so, NULL);
         count_launch();
     } else {
-        k4_flat<128, 8, false, false><<<p.NB, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so, NULL);  // 64 regs, 32 warps/SM
+        k4_flat<128, 8, false, false><<<grid4, 128, 0, st>>>(p, counts, list, d_bits_out, hdr, so, NULL);  // 64 regs, 32 warps/SM
         count_launch();
     }
     CK(cudaGetLastError());
