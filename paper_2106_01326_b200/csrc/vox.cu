@@ -32,6 +32,7 @@ struct Params {
     const int4* verts4;  // fused lattice path: K0's 16-byte copy of the vertices (x, y, z, 0) in the workspace, else NULL
     const unsigned char* keep;  // lattice input (vox_lattice): bit q of keep[cell] = tet q of the cell is present
     int lcx, lcy, lcz;          // cells per axis of the lattice input; lcx == 0: explicit tets
+    int fused;                  // lattice input takes the fused path (lattice_fused)
     i64 T;
     i64 V;
     int batch;
@@ -114,9 +115,10 @@ static inline void count_launch() { __atomic_fetch_add(&g_launches, 1ull, __ATOM
 struct WsLayout {
     size_t hdr, slab, counts, cursor, big, range, list, fixed_end;
 };
-// lattice input: per mesh 2 * ((cx+1) + (cy+1) + (cz+1)) ints of vertex-plane bounds (k0_slabs), else nothing
+// fused lattice path: per mesh 2 * ((cx+1) + (cy+1) + (cz+1)) ints of vertex-plane bounds (k0_slabs), else nothing
+// (the binned paths keep the layout a pipe sized for them)
 static size_t slab_ints(const Params& p) {
-    return p.lcx ? (size_t)p.batch * 2 * ((size_t)p.lcx + p.lcy + p.lcz + 3) : 0;
+    return p.fused ? (size_t)p.batch * 2 * ((size_t)p.lcx + p.lcy + p.lcz + 3) : 0;
 }
 static WsLayout ws_layout(const Params& p) {
     WsLayout L;
@@ -1557,11 +1559,19 @@ extern "C" int vox_set_tile(vox_ctx* ctx, int ty, int tz) {
     return VOX_OK;
 }
 
+// lattice input takes the fused path (K0 + K4, no binning) unless variant 1 asks for the binned one or the lattice
+// is beyond what k0_slabs / the candidate queue were sized for
+static bool lattice_fused(const vox_ctx* ctx) {
+    const Params& p = ctx->p;
+    return p.lcx > 0 && ctx->variant == 0 && p.lcx <= 4096 && p.lcy <= 4096 && p.lcz <= 4096 && p.V < (1ll << 28);
+}
+
 extern "C" int vox_set_variant(vox_ctx* ctx, int variant) {
     // 0: default.  1: lattice input goes through the binning passes K1-K3 like a tet array (cross-check of the
     // fused lattice path; no effect on explicit tets)
     if (!ctx || (variant != 0 && variant != 1)) return VOX_EINVAL;
     ctx->variant = variant;
+    ctx->p.fused = lattice_fused(ctx) ? 1 : 0;
     return VOX_OK;
 }
 
@@ -1579,6 +1589,7 @@ extern "C" int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const i
     ctx->p.off = (ctx->p.batch > 1) ? (const i64*)d_tet_offsets : NULL;
     ctx->p.keep = NULL;
     ctx->p.lcx = ctx->p.lcy = ctx->p.lcz = 0;
+    ctx->p.fused = 0;
     if (!ctx->tile_user) auto_tile(ctx->p, T);
     ctx->have_tets = true;
     ctx->pairs_planned = -1;
@@ -1597,19 +1608,13 @@ extern "C" int vox_lattice(vox_ctx* ctx, const int32_t* d_verts, int cx, int cy,
     p.lcx = cx; p.lcy = cy; p.lcz = cz;
     p.V = V;
     p.T = 6 * cells;
+    p.fused = lattice_fused(ctx) ? 1 : 0;
     // (T counts the absent tets too: a carved lattice keeps a fraction, a third is assumed for the tile choice; larger
     //  tiles also mean a thinner rim of candidate cells per tile on the fused path)
     if (!ctx->tile_user) auto_tile(p, p.T / 3);
     ctx->have_tets = true;
     ctx->pairs_planned = -1;
     return VOX_OK;
-}
-
-// lattice input takes the fused path (K0 + K4, no binning) unless variant 1 asks for the binned one or the lattice
-// is beyond what k0_slabs / the candidate queue were sized for
-static bool lattice_fused(const vox_ctx* ctx) {
-    const Params& p = ctx->p;
-    return p.lcx > 0 && ctx->variant == 0 && p.lcx <= 4096 && p.lcy <= 4096 && p.lcz <= 4096 && p.V < (1ll << 28);
 }
 
 extern "C" size_t vox_grid_words(const vox_ctx* ctx) {
