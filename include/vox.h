@@ -98,7 +98,7 @@ int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const int32_t* d_t
  * the definition's).  Its workspace is the header, 8*(cx+cy+cz+3) bytes per mesh and a 16-byte copy of every vertex
  * (vox_workspace_bytes);
  * vox_status then reports culled = 0 (slivers and degenerate tets are skipped per tile, not counted per tet).
- * Lattices beyond 4096 cells per axis or 2^28 vertices, and vox_set_variant(ctx, 1), take the binning passes
+ * Lattices beyond 4096 cells per axis, 2^28 vertices or 65535 meshes, and vox_set_variant(ctx, 1), take the binning passes
  * (vox_status then counts only present tets as culled).  vox_plan always runs the binning count. */
 int vox_lattice(vox_ctx* ctx, const int32_t* d_verts, int cx, int cy, int cz, const uint8_t* d_keep);
 

@@ -1563,7 +1563,8 @@ extern "C" int vox_set_tile(vox_ctx* ctx, int ty, int tz) {
 // is beyond what k0_slabs / the candidate queue were sized for
 static bool lattice_fused(const vox_ctx* ctx) {
     const Params& p = ctx->p;
-    return p.lcx > 0 && ctx->variant == 0 && p.lcx <= 4096 && p.lcy <= 4096 && p.lcz <= 4096 && p.V < (1ll << 28);
+    return p.lcx > 0 && ctx->variant == 0 && p.lcx <= 4096 && p.lcy <= 4096 && p.lcz <= 4096 && p.V < (1ll << 28) &&
+           p.batch <= 65535;  // (k0_slabs: shared-memory z table, gridDim.z = batch; queue entries are v0 << 3 | q)
 }
 
 extern "C" int vox_set_variant(vox_ctx* ctx, int variant) {

@@ -527,6 +527,41 @@ def test_randomized_magnitudes_straddle_the_int32_limit():
     assert 0.2 * pairs < large < 0.8 * pairs
 
 
+def test_fast_setup_fit_test_is_straddled():
+    """Round 2's fast plane setup is taken when 24*dx*dy*dz/g + 16*max(dy*dz*sx, dx*dz*sy, dx*dy*sz) < 2*10^9 (d = the tet's
+    lattice bbox extents); everything else goes through the range-checked general setup.  Random tets whose
+    extents sit around that bound, on power-of-two pitches (cubic and anisotropic), so that both routes -- and the
+    general path's int32 / int64 split behind it -- meet in the same tiles.  The inequality is restated here only to
+    assert that both sides occur; the expected grid is the oracle's."""
+    fast = slow = 0
+    for seed, (n, Ex) in enumerate([((128, 128, 128), (65536,) * 3), ((256, 256, 256), (16384,) * 3),
+                                    ((128, 64, 32), (65536, 65536, 65536)), ((256, 256, 256), (1 << 20,) * 3)]):
+        rng = np.random.default_rng(7000 + seed)
+        h = [e // k for e, k in zip(Ex, n)]
+        g = int(np.gcd.reduce(h))
+        sx, sy, sz = (x // g for x in h)
+        # extent at which a cubic bbox meets the bound: 24 d^3 / g + 16 d^2 s = 2e9
+        d0 = int(min((2e9 * g / 24) ** (1 / 3), 30000))
+        verts, tets = [], []
+        for _ in range(400):
+            size = int(d0 * 2 ** rng.uniform(-0.2, 1.4))
+            c = np.array([rng.integers(0, e + 1) for e in Ex])
+            pts = np.clip(c + rng.integers(-size // 2, size // 2 + 1, (4, 3)), 0, np.array(Ex))
+            d = pts.max(0) - pts.min(0)
+            if max(d) < 32768 and 24.0 * d[0] * d[1] * d[2] / g + 16.0 * max(d[1] * d[2] * sx, d[0] * d[2] * sy, d[0] * d[1] * sz) < 2.0e9:
+                fast += 1
+            else:
+                slow += 1
+            b = len(verts)
+            verts += pts.tolist()
+            tets.append([b, b + 1, b + 2, b + 3])
+        m = Mesh(f"fit{seed}", np.array(verts, dtype=np.int32), np.array(tets, dtype=np.int32), n, Ex)
+        exp = cpu_voxelize(m)
+        assert_same(gpu_voxelize(m), exp, f"fit-test straddle {n} {Ex}")
+        assert_same(gpu_voxelize(m, tile=(8, 8)), exp, f"fit-test straddle {n} {Ex} tile 8x8")
+    assert fast > 400 and slow > 400, (fast, slow)
+
+
 def test_more_oversized_tets_than_the_handover_list_holds():
     """Tets whose tile range exceeds 64 tiles are handed from K1 to K2's CTA through a 4096-entry list; with 5000 of
     them the rest falls back to the per-thread walk.  Both routes in one mesh, plus small tets."""

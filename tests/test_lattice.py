@@ -35,12 +35,26 @@ def _cases():
     out.append(("aniso", Mesh("aniso", v, t, (96, 40, 24), (96 * 8, 40 * 8, 24 * 8)), (5, 3, 7)))
     b = meshgen.make_config("cfg3_small")                    # a batch of 4 meshes on the same 24^3 lattice
     out.append(("cfg3_small", b, b.cells))
+    # pitch 12 (not a power of two: the division forms of the box and the general plane setup), ragged grid
+    xs, ys, zs = (np.rint(np.linspace(0, e, n + 1)).astype(np.int64) for e, n in ((64 * 12, 7), (40 * 12, 5), (24 * 12, 4)))
+    v, t = kuhn_mesh(xs, ys, zs, 0.2, rng)
+    t = t[rng.random(len(t)) < 0.7]
+    out.append(("nonpow2", Mesh("nonpow2", v, t, (64, 40, 24), (64 * 12, 40 * 12, 24 * 12)), (7, 5, 4)))
+    # sub-voxel cells: 40^3 cells on a 32^3 grid (0.8 voxel per cell): most tets hold no sample (culled per tile on
+    # the fused path), a tile's index box holds tens of thousands of cells
+    c = _uniform_corners(40)
+    v, t = kuhn_mesh(c, c, c, 0.2, rng)
+    t = t[rng.random(len(t)) < 0.5]
+    out.append(("subvoxel", Mesh("subvoxel", v, t, (32, 32, 32)), (40, 40, 40)))
+    # giant cells: 2^3 cells on a 128^3 grid (every tile sees all 48 tets; int64 large path)
+    g = meshgen.make_config("s1")
+    out.append(("giant", Mesh("giant", g.verts, g.tets[::2].copy(), (128, 128, 128)), (2, 2, 2)))
     return out
 
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("variant", [0, 1], ids=["fused", "binned"])
-@pytest.mark.parametrize("idx", range(5))
+@pytest.mark.parametrize("idx", range(8))
 def test_gpu_lattice_input_matches_oracle(idx, variant):
     """variant 0: the fused lattice path (K0 slabs + tiles enumerating their own candidate cells, no K1-K3);
     variant 1: the same input through the binning passes.  Both must give the oracle's grid and count the same
