@@ -444,23 +444,22 @@ __global__ void __launch_bounds__(256) k3_scatter(Params p, const uint2* __restr
     // (tried, round 2: one atomic per (tet, tile) with up to 8 in flight per thread instead of the lockstep aggregation --
     //  2-3.5x slower, 0.15 against 0.072 ms on cfg4, 0.32 against 0.092 on the 10^7-tet mesh: the cursors of a tile are hot
     //  addresses and the number of atomics, not their latency, is what binds)
-    // warp-aggregated cursor bump (same stepping as K1): one atomic per distinct tile per step,
-    // the lanes of a group take consecutive slots (order inside a tile list is irrelevant: OR)
+    // warp-aggregated cursor bump (same stepping as K1): one atomic per distinct tile per step, the lanes of a group
+    // take consecutive slots (order inside a tile list is irrelevant: OR).  TWO steps per trip: the kernel is bound by
+    // the round trip of the returning atomics, and most tets touch one or two tiles, so the atomics of a lane's next
+    // tile are put in flight together with those of its current one.
     const int lane = threadIdx.x & 31;
+    const u32 lt = (1u << lane) - 1u;
     for (;;) {
-        const unsigned act = __ballot_sync(0xFFFFFFFFu, live);
-        if (!act) break;
+        const unsigned actA = __ballot_sync(0xFFFFFFFFu, live);
+        if (!actA) break;
+        u32 bA = 0, bB = 0;
+        unsigned peersA = 0, peersB = 0;
+        bool liveB = false;
         if (live) {
-            const u32 b = ((((u32)m * p.nbz + cz) * p.nby + cy) * p.nbx) + cx;
-            VOX_CHECK(b < p.NB, CK_K3_TILE);
-            const unsigned peers = __match_any_sync(act, b);
-            const int leader = __ffs(peers) - 1;
-            u32 base = 0;
-            if (lane == leader) base = atomicAdd(cursor + b, (u32)__popc(peers));
-            base = __shfl_sync(peers, base, leader);
-            const u32 pos = base + (u32)__popc(peers & ((1u << lane) - 1u));
-            if (pos < p.cap) list[pos] = (u32)t;
-            else hdr[H_OVERFLOW] = 1;
+            bA = ((((u32)m * p.nbz + cz) * p.nby + cy) * p.nbx) + cx;
+            VOX_CHECK(bA < p.NB, CK_K3_TILE);
+            peersA = __match_any_sync(actA, bA);
             if (++cx > b1x) {
                 cx = b0x;
                 if (++cy > b1y) {
@@ -468,6 +467,36 @@ __global__ void __launch_bounds__(256) k3_scatter(Params p, const uint2* __restr
                     live = (++cz <= b1z);
                 }
             }
+            liveB = live;
+        }
+        const unsigned actB = __ballot_sync(0xFFFFFFFFu, liveB);
+        if (liveB) {
+            bB = ((((u32)m * p.nbz + cz) * p.nby + cy) * p.nbx) + cx;
+            VOX_CHECK(bB < p.NB, CK_K3_TILE);
+            peersB = __match_any_sync(actB, bB);
+            if (++cx > b1x) {
+                cx = b0x;
+                if (++cy > b1y) {
+                    cy = b0y;
+                    live = (++cz <= b1z);
+                }
+            }
+        }
+        // both groups' atomics in flight before either result is used
+        u32 baseA = 0, baseB = 0;
+        if (peersA && lane == __ffs(peersA) - 1) baseA = atomicAdd(cursor + bA, (u32)__popc(peersA));
+        if (peersB && lane == __ffs(peersB) - 1) baseB = atomicAdd(cursor + bB, (u32)__popc(peersB));
+        if (peersA) {
+            baseA = __shfl_sync(peersA, baseA, __ffs(peersA) - 1);
+            const u32 pos = baseA + (u32)__popc(peersA & lt);
+            if (pos < p.cap) list[pos] = (u32)t;
+            else hdr[H_OVERFLOW] = 1;
+        }
+        if (peersB) {
+            baseB = __shfl_sync(peersB, baseB, __ffs(peersB) - 1);
+            const u32 pos = baseB + (u32)__popc(peersB & lt);
+            if (pos < p.cap) list[pos] = (u32)t;
+            else hdr[H_OVERFLOW] = 1;
         }
     }
 }
@@ -587,17 +616,19 @@ __device__ __forceinline__ bool span_plane(const Params& p, int* rec, int pos, i
     int mx = (int)(0u - (u32)nx * (u32)p.sx), my = (int)(0u - (u32)ny * (u32)p.sy), mz = (int)(0u - (u32)nz * (u32)p.sz);
     const i64 C = (i64)nx * rx + (i64)ny * ry + (i64)nz * rz;
     const i64 g64 = (C >> p.g_shift) + (i64)mx * x0 + (i64)my * y0 + (i64)mz * z0;  // G at the box origin
-    ok = ok && ((u64)(g64 + (1ll << 30)) < (1ull << 31));                          // |g0| <= 2^30
+    ok = ok && ((u64)(g64 + (1ll << 31) - 1) < (1ull << 32) - 2);                  // |g0| < 2^31 (acc below bounds it further)
     int g0 = (int)g64;
     if (mx > 0) { mx = (int)(0u - (u32)mx); my = (int)(0u - (u32)my); mz = (int)(0u - (u32)mz); g0 = ~g0; }  // lo-type: Q = -G - 1
-    // scale: 4, so that |mx| >= 4 and the reciprocal ceil(2^32 / |mx|) fits int32; a plane with mx == 0 does
+    // scale: 4 (when |mx| < 4), so that |mx| >= 4 and the reciprocal ceil(2^32 / |mx|) fits int32; a plane with mx == 0 does
     // not depend on x and only gates the row: stored as r' = 64*G + 63 with inv = 2^31 - 1, for which span_bound
     // gives c0 = floor(r'/2 - r'/2^32) >= 31 when r' >= 63 (G >= 0: not binding, x1' <= 31) and b = c0 - 1 <= -2
     // when r' <= -1 (G < 0: empty row).
     // (every x-dependent plane is scaled by 4, not "2, or 4 when |mx| == 1": ptxas 12.9 at -O1 and above folds the
     //  test `mx == -1` on the negated absolute value to false -- SASS keeps only the cases 1 and 6 -- which the
     //  parity suite caught twice)
-    const int sh = (mx == 0) ? 6 : 2;
+    // (general path, round 2: a plane whose |mx| is already >= 4 is not scaled at all -- two more bits of headroom before
+    //  a pair has to take the int64 path: the Table-1 mesh of 10^5 tets had 41 043 such pairs)
+    const int sh = (mx == 0) ? 6 : (((u32)0 - (u32)mx) >= 4u ? 0 : 2);
     // every row value r of the box and r +- 2*mx (span_bound's product and check) must fit int32 after scaling
     u64 acc = (u64)(u32)abs(g0) + 2ull * (0u - (u32)mx);
     acc += (u64)(u32)wy * (u32)abs(my);

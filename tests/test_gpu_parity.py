@@ -501,9 +501,9 @@ def test_randomized_jobs_match_oracle(block):
 
 
 def test_randomized_magnitudes_straddle_the_int32_limit():
-    """Random tets of 2^4..2^13.5 lattice units on lattices of extent 2^14..2^20: about half of the (tet, tile)
-    pairs fit the int32 span path and half take the int64 large path, so the hand-over bound is exercised from
-    both sides."""
+    """Random tets of 2^4..2^14.5 lattice units on lattices of extent 2^14..2^20: a good part of the (tet, tile)
+    pairs fits the int32 span path and a good part takes the int64 large path (plane values beyond int32, or bbox
+    extents beyond 2^15), so the hand-over bound is exercised from both sides."""
     import paper_2106_01326_b200 as pkg
 
     large = pairs = 0
@@ -513,7 +513,7 @@ def test_randomized_magnitudes_straddle_the_int32_limit():
         Ex = 1 << int(rng.integers(14, 21))
         verts, tets = [], []
         for _ in range(int(rng.integers(5, 60))):
-            size = int(2 ** rng.uniform(4, 13.5))
+            size = int(2 ** rng.uniform(4, 14.5))
             c = rng.integers(0, Ex + 1, 3)
             pts = np.clip(c + rng.integers(-size // 2, size // 2 + 1, (4, 3)), 0, Ex)
             b = len(verts)
@@ -524,7 +524,7 @@ def test_randomized_magnitudes_straddle_the_int32_limit():
         assert_same(gpu_voxelize(m, tile=tile), cpu_voxelize(m), f"magnitude seed {seed} n {n} E {Ex} tile {tile}")
         large += pkg.voxelize.last_status["large_pairs"]
         pairs += pkg.voxelize.last_status["pairs"]
-    assert 0.2 * pairs < large < 0.8 * pairs
+    assert 0.1 * pairs < large < 0.9 * pairs, (large, pairs)
 
 
 def test_fast_setup_fit_test_is_straddled():
