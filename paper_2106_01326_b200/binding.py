@@ -234,6 +234,24 @@ class Voxelizer:
         )
         return out
 
+    def capture(self, out, steps=1, stream=None):
+        """CUDA graph of `steps` vox_run calls into `out` (vox_run only enqueues: no sync, no allocation, so it can be
+        stream-captured).  Returns the torch.cuda.CUDAGraph; replay() re-runs the step(s) on the mesh, workspace and
+        output bound now.  Worth ~6-8 us per step: it removes the launch gaps between the memset and the four kernels,
+        which is a sixth of a step on the smallest configs and nothing on the large ones."""
+        torch = _torch_cuda()
+        if self._ws is None:
+            self.alloc_workspace()
+        stream = stream or torch.cuda.Stream()
+        with torch.cuda.stream(stream):
+            self.run(out, stream)  # warm-up outside the capture
+            stream.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                for _ in range(int(steps)):
+                    self.run(out, stream)
+        return g
+
     @property
     def tile_shape(self):
         """dict(ty, tz, nbx, nby, nbz): the binning tile (32 x ty x tz voxels) and tiles per axis."""

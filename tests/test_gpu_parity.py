@@ -106,6 +106,31 @@ def test_unknown_kernel_variant_is_refused():
         pkg.Pipe((32, 32, 32), depth=1, max_V=4, max_T=1, variant=2)
 
 
+def test_graph_replay_of_a_step_matches_oracle():
+    """vox_run only enqueues, so a step can be captured into a CUDA graph and replayed (Voxelizer.capture)."""
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    for name in ("cfg2", "cfg3_small"):
+        m = CASES[name]()
+        exp = cpu_voxelize(m)
+        vz = pkg.Voxelizer(m.grid, m.extent, m.batch)
+        off = torch.from_numpy(m.tet_offsets).cuda() if m.batch > 1 else None
+        vz.set_tets(torch.from_numpy(m.verts).cuda(), torch.from_numpy(m.tets).cuda(), off)
+        vz.plan()
+        nx, ny, nz = m.grid
+        out = torch.empty((m.batch, nz, ny, nx // 32), dtype=torch.int32, device="cuda")
+        g = vz.capture(out, steps=2)
+        for _ in range(3):
+            out.fill_(-1)                      # stale bits must be overwritten by every replay
+            g.replay()
+            torch.cuda.synchronize()
+            assert_same(out.cpu().numpy().view(np.uint32), exp, f"graph replay {name}")
+        assert vz.status()["pairs"] > 0
+        vz.close()
+
+
 def test_estimated_workspace_path():
     m = CASES["cfg2"]()
     assert_same(gpu_voxelize(m, exact_plan=False), cpu_voxelize(m), "cfg2 without vox_plan")
