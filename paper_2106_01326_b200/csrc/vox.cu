@@ -1010,15 +1010,13 @@ __device__ __forceinline__ void lane_row(const LaneRec& L, int rr, int img_strid
     const u32 saddr = (u32)L.B.x + 4u * (u32)(zz * img_stride + yy);
     VOX_CHECK(rr >= 0 && rr < L.A.w && yy >= 0 && yy < L.A.z && zz >= 0 && zz <= 31, CK_K4_ROWS);
     VOX_CHECK(saddr >= img_lo && saddr < img_hi && (saddr & 3u) == 0, CK_K4_ROWADDR);
-    // branch-free: PTX shifts clamp at 32, so n <= 0 gives word 0 and the OR is a no-op
+    // branch-free: the word is a mask of max(n, 0) bits from bit lower + 1 + x0 (BMSK); n <= 0 gives 0 and the OR is a no-op
+    const int width = max(n, 0), pos = lower + L.A.x;
     asm volatile(
-        "{\n\t.reg .b32 m, s;\n\t"
-        "sub.s32 s, 32, %1;\n\t"
-        "shr.b32 m, 0xFFFFFFFF, s;\n\t"
-        "add.s32 s, %2, %3;\n\t"
-        "shl.b32 m, m, s;\n\t"
+        "{\n\t.reg .b32 m;\n\t"
+        "bmsk.clamp.b32 m, %1, %2;\n\t"
         "red.shared.or.b32 [%0], m;\n\t}"
-        ::"r"(saddr), "r"(n), "r"(lower), "r"(L.A.x)
+        ::"r"(saddr), "r"(pos), "r"(width)
         : "memory");
 }
 
