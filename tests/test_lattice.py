@@ -176,3 +176,34 @@ def test_gpu_random_lattices_match_oracle(block):
         assert pairs[0] == pairs[1], (seed, pairs)
         done += 1
     assert done >= 8
+
+
+@pytest.mark.gpu
+def test_gpu_fused_lattice_with_a_huge_index_box():
+    """160^3 sub-voxel cells on a 32^3 grid with one 32^3 tile: the tile's index box holds 4.1 M cells, beyond the 2^21
+    up to which the fused path decodes a cell with float reciprocals -- the integer-division branch of the
+    enumeration.  8 % of the tets kept; nearly all of them hold no sample and are skipped per tile."""
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    rng = np.random.default_rng(99)
+    C = 160
+    c = _uniform_corners(C)
+    v, t = kuhn_mesh(c, c, c, 0.2, rng)
+    t = t[rng.random(len(t)) < 0.08]
+    m = Mesh("hugebox", v, t, (32, 32, 32))
+    exp = oracle.voxelize(m.verts, m.tets, m.grid, m.extent)
+    keep = meshgen.lattice_form(m, (C, C, C))
+    dv, dk = torch.from_numpy(m.verts).cuda(), torch.from_numpy(keep).cuda()
+    pairs = {}
+    for tile in ((32, 32), (8, 8)):
+        for variant in (0, 1):
+            vz = pkg.Voxelizer(m.grid, m.extent, 1, tile=tile, variant=variant)
+            vz.set_lattice(dv, (C, C, C), dk)
+            vz.plan()
+            got = vz.run().cpu().numpy().view(np.uint32)
+            pairs[(tile, variant)] = vz.status()["pairs"]
+            vz.close()
+            assert np.array_equal(got, exp), f"tile {tile} variant {variant}: {(got != exp).sum()} words differ"
+        assert pairs[(tile, 0)] == pairs[(tile, 1)] > 0
