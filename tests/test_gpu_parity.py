@@ -587,6 +587,28 @@ def test_fast_setup_fit_test_is_straddled():
     assert fast > 400 and slow > 400, (fast, slow)
 
 
+def test_more_meshes_than_griddim_z_holds():
+    """K4 runs on a 3-D grid (tiles x, tiles y, tiles z * batch) when that fits gridDim and on a 1-D grid otherwise:
+    66 000 meshes of 32 x 8 x 8 voxels (one tile each) take the 1-D launch.  Every third mesh holds a tet, the rest are
+    empty."""
+    B = 66000
+    rng = np.random.default_rng(66)
+    verts, tets, off = [], [], [0]
+    for m_ in range(B):
+        if m_ % 3 == 0:
+            pts = rng.integers(0, [64 * 32 + 1, 64 * 8 + 1, 64 * 8 + 1], (4, 3))
+            b = len(verts)
+            verts += pts.tolist()
+            tets.append([b, b + 1, b + 2, b + 3])
+        off.append(len(tets))
+    m = Mesh("manymeshes", np.array(verts, dtype=np.int32), np.array(tets, dtype=np.int32), (32, 8, 8), (64 * 32, 64 * 8, 64 * 8),
+             tet_offsets=np.array(off, dtype=np.int64))
+    assert m.batch == B
+    exp = cpu_voxelize(m)
+    assert exp.any()
+    assert_same(gpu_voxelize(m), exp, "66000 meshes")
+
+
 def test_more_oversized_tets_than_the_handover_list_holds():
     """Tets whose tile range exceeds 64 tiles are handed from K1 to K2's CTA through a 4096-entry list; with 5000 of
     them the rest falls back to the per-thread walk.  Both routes in one mesh, plus small tets."""
