@@ -18,7 +18,8 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 SUBSET = ("small_configs or sparse_output or ragged or oversized or max_extent or straddle or randomized_jobs or "
           "unit_and_zero or random_soup or all_tets_culled or empty_mesh or p1_single or pipe_stream or "
-          "gpu_lattice_input_matches or lattice_through_the_pipe or batched_lattice")
+          "gpu_lattice_input_matches or lattice_through_the_pipe or batched_lattice or fit_test or more_meshes or "
+          "random_lattices or huge_index or graph_replay")
 
 
 def _checked_lib():
