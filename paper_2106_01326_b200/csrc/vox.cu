@@ -164,16 +164,18 @@ struct Tet {
 
 // Lattice input (include/vox.h "vox_lattice"): tet t = 6*cell + q of cell (i,j,k) walks from the cell's low corner
 // along the axes of the q-th permutation of (x,y,z) in lexicographic order; vertex id = (i*(cy+1) + j)*(cz+1) + k.
-__device__ __forceinline__ int4 lattice_ids(const Params& p, i64 t) {
-    const int q = (int)(t % 6);
-    i64 c = t / 6;
-    const i64 cells = (i64)p.lcx * p.lcy * p.lcz;
-    const int mesh = (int)(c / cells);  // batch: mesh m owns cells [m*cells, (m+1)*cells) and its own vertex block
-    c -= mesh * cells;
-    const int k = (int)(c % p.lcz);
-    c /= p.lcz;
-    const int j = (int)(c % p.lcy);
-    const int i = (int)(c / p.lcy);
+__device__ __forceinline__ int4 lattice_ids(const Params& p, i64 t64) {
+    // 32-bit arithmetic throughout: T = 6 * cells * batch <= 0xFFFFFFF0 (vox_lattice)
+    const u32 t = (u32)t64;
+    const int q = (int)(t % 6u);
+    u32 c = t / 6u;
+    const u32 cells = (u32)p.lcx * (u32)p.lcy * (u32)p.lcz;
+    const int mesh = (p.batch == 1) ? 0 : (int)(c / cells);  // mesh m owns cells [m*cells, (m+1)*cells) and its own vertex block
+    c -= (u32)mesh * cells;
+    const int k = (int)(c % (u32)p.lcz);
+    c /= (u32)p.lcz;
+    const int j = (int)(c % (u32)p.lcy);
+    const int i = (int)(c / (u32)p.lcy);
     const int sz = 1, sy = p.lcz + 1, sx = (p.lcy + 1) * (p.lcz + 1);
     const int v0 = mesh * (p.lcx + 1) * sx + (i * (p.lcy + 1) + j) * (p.lcz + 1) + k;
     // permutations of (x,y,z), lexicographic: xyz xzy yxz yzx zxy zyx
@@ -215,7 +217,7 @@ __device__ __forceinline__ void axis_range(int a, int b, int c, int d, int h, in
 
 __device__ __forceinline__ int mesh_of(const Params& p, i64 t) {
     if (p.batch == 1) return 0;
-    if (p.lcx) return (int)(t / (6ll * p.lcx * p.lcy * p.lcz));  // lattice input: equal blocks per mesh
+    if (p.lcx) return (int)((u32)t / (6u * (u32)p.lcx * (u32)p.lcy * (u32)p.lcz));  // lattice input: equal blocks per mesh
     int lo = 0, hi = p.batch;  // off[lo] <= t < off[hi]
     while (hi - lo > 1) {
         int mid = (lo + hi) >> 1;
@@ -236,7 +238,7 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
     uint2 r = make_uint2(RANGE_CULLED, 0u);
     int m = 0;
     int b0x = 0, b1x = -1, b0y = 0, b1y = -1, b0z = 0, b1z = -1;
-    const bool present = (t < p.T) && (!p.lcx || ((__ldg(p.keep + t / 6) >> (int)(t % 6)) & 1));
+    const bool present = (t < p.T) && (!p.lcx || ((__ldg(p.keep + (u32)t / 6u) >> (int)((u32)t % 6u)) & 1));
     if (t < p.T && !present) range[t] = r;  // lattice input: the cell does not keep this tet
     if (present) {
         Tet q = load_tet(p, t);
