@@ -239,7 +239,7 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
     int m = 0;
     int b0x = 0, b1x = -1, b0y = 0, b1y = -1, b0z = 0, b1z = -1;
     const bool present = (t < p.T) && (!p.lcx || ((__ldg(p.keep + (u32)t / 6u) >> (int)((u32)t % 6u)) & 1));
-    if (t < p.T && !present) range[t] = r;  // lattice input: the cell does not keep this tet
+    // (lattice input: a tet its cell does not keep gets no range entry -- K3 looks at the keep bit first)
     if (present) {
         Tet q = load_tet(p, t);
         int x0, x1, y0, y1, z0, z1;
@@ -433,7 +433,7 @@ __global__ void __launch_bounds__(256) k3_scatter(Params p, const uint2* __restr
     i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
     bool live = false;
     int b0x = 0, b0y = 0, b1x = 0, b1y = 0, b1z = 0, cx = 0, cy = 0, cz = 0, m = 0;
-    if (t < p.T) {
+    if (t < p.T && (!p.lcx || ((__ldg(p.keep + (u32)t / 6u) >> (int)((u32)t % 6u)) & 1))) {
         const uint2 r = range[t];
         if (r.x != RANGE_CULLED && !(r.x & RANGE_BIG)) {  // (oversized tets were scattered by K2)
             live = true;
