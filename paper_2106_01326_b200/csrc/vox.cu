@@ -199,10 +199,16 @@ __device__ __forceinline__ Tet load_tet(const Params& p, i64 t) {
 
 // 6V = det[B-A; C-A; D-A]  (Lemma 1.1)
 __device__ __forceinline__ i64 six_volume(const Tet& q) {
-    i64 ux = q.bx - q.ax, uy = q.by - q.ay, uz = q.bz - q.az;
-    i64 vx = q.cx - q.ax, vy = q.cy - q.ay, vz = q.cz - q.az;
-    i64 wx = q.dx - q.ax, wy = q.dy - q.ay, wz = q.dz - q.az;
-    return ux * (vy * wz - vz * wy) - uy * (vx * wz - vz * wx) + uz * (vx * wy - vy * wx);
+    const int ux = q.bx - q.ax, uy = q.by - q.ay, uz = q.bz - q.az;
+    const int vx = q.cx - q.ax, vy = q.cy - q.ay, vz = q.cz - q.az;
+    const int wx = q.dx - q.ax, wy = q.dy - q.ay, wz = q.dz - q.az;
+    // every edge component below 2^15 (the usual case): v x w fits int32, only the final dot product is 64-bit
+    const int big = abs(ux) | abs(uy) | abs(uz) | abs(vx) | abs(vy) | abs(vz) | abs(wx) | abs(wy) | abs(wz);
+    if (big < 32768) {
+        const int cx = vy * wz - vz * wy, cy = vz * wx - vx * wz, cz = vx * wy - vy * wx;
+        return (i64)ux * cx + (i64)uy * cy + (i64)uz * cz;
+    }
+    return (i64)ux * ((i64)vy * wz - (i64)vz * wy) - (i64)uy * ((i64)vx * wz - (i64)vz * wx) + (i64)uz * ((i64)vx * wy - (i64)vy * wx);
 }
 
 // closed voxel-index range of centres h*i + h/2 inside [lo, hi], clamped to the grid
