@@ -128,6 +128,41 @@ int vox_run(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes,
  * non-empty bricks}. */
 int vox_status(vox_ctx* ctx, void* cuda_stream, const void* d_workspace, int64_t stats_out[4]);
 
+/* vox_run for callers that cannot allocate device memory.
+ *
+ * vox_run leaves the workspace to the caller, which normally means a cudaMalloc (or a framework tensor).  Some
+ * callers of this library have no way to make one: a plug-in inside a host application whose own pool has
+ * already claimed the whole GPU and which hands the plug-in nothing but its input and output buffers; a
+ * service loop that must not stall its other streams (cudaMalloc and cudaFree synchronise the device); code
+ * that runs while some other thread of the process is capturing a CUDA graph in the global capture mode,
+ * where an allocation call is an error and ruins that capture.  For them the library carries its own
+ * workspace: VOX_NOALLOC_SCRATCH_BYTES of device memory inside the library image, present on every GPU that
+ * loads libvox.so from then until the process exits, whether or not this call is ever used.
+ *
+ * The call is vox_run with that built-in workspace: same kernels, same result, every word of d_bits_out
+ * written.  The caller still passes the inputs (vox_tets / vox_lattice) and the output grid.  It calls no
+ * cudaMalloc, cudaFree or any routine that allocates; it enqueues a memset and the kernels on `cuda_stream`.
+ *
+ *   Limit.   vox_workspace_bytes(ctx) must not exceed VOX_NOALLOC_SCRATCH_BYTES (4 MiB: roughly 24 bytes
+ *            per tet plus 8 per tile, i.e. meshes up to ~150 000 tets on grids up to ~256^3; config 2 of
+ *            BASELINE.json needs 1.9 MB).  Anything larger is refused with VOX_EWORKSPACE before any GPU
+ *            work, and vox_last_error(ctx) says how many bytes were needed and how many there are.
+ *   Set-up.  The first call on each device looks up that device's address of the built-in array
+ *            (the device that is current at the call, which must be the one `cuda_stream` belongs to) and
+ *            remembers it.  Make this first call before any stream capture begins.  Up to 64 devices.
+ *   Sharing. There is ONE such array per device and every call on that device uses it, whatever the ctx,
+ *            stream or thread.  Each call clears the counters it needs to start at zero itself, so stale
+ *            contents from the previous call never matter; but two calls whose GPU work can overlap (different
+ *            streams, no dependency between them) race on the array and both results are undefined.  Order
+ *            them on one stream or with events.
+ *   Status.  stats_out == NULL: enqueue only, as vox_run.  stats_out != NULL: the call then WAITS for the
+ *            stream and fills stats_out like vox_status ({pairs, culled tets, large-path pairs, non-empty
+ *            tiles}); it returns VOX_EWORKSPACE if the mesh produced more (tet, tile) pairs than the array
+ *            had room for (tets were dropped: the grid is incomplete).  The estimate behind
+ *            vox_workspace_bytes is not an upper bound, so pass stats_out at least once per kind of mesh. */
+#define VOX_NOALLOC_SCRATCH_BYTES (4u << 20)
+int vox_run_noalloc(vox_ctx* ctx, void* cuda_stream, uint32_t* d_bits_out, int64_t stats_out[4]);
+
 /* Sparse (two-level) output.  "voxels are often calculated and stored in
  * octree data formats"; the binning tiles give a two-level store for free:
  * a table with one word per tile plus the row words of the MIXED tiles only.

@@ -19,8 +19,11 @@ EXPORTS = [
     "vox_pipe_bind", "vox_pipe_submit", "vox_pipe_wait", "vox_pipe_last_error",
     "vox_tile_shape", "vox_run_sparse", "vox_sparse_status", "vox_pipe_submit_sparse", "vox_pipe_tile_shape",
     "vox_pipe_reserve_pairs", "vox_occupancy", "vox_lattice", "vox_pipe_submit_lattice", "vox_kernel_launches",
-    "vox_debug_check_status",
+    "vox_debug_check_status", "vox_run_noalloc",
 ]
+
+
+NOALLOC_SCRATCH_BYTES = 4 << 20  # include/vox.h VOX_NOALLOC_SCRATCH_BYTES
 
 
 class VoxError(RuntimeError):
@@ -85,6 +88,7 @@ def load_library():
         "vox_pipe_submit_lattice": (i32, [vp, vp, i32, i32, i32, vp, vp, vp, i64, ctypes.POINTER(i64)]),
         "vox_kernel_launches": (ctypes.c_uint64, []),
         "vox_debug_check_status": (i32, [ctypes.POINTER(ctypes.c_uint32)]),
+        "vox_run_noalloc": (i32, [vp, vp, vp, ctypes.POINTER(i64)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -233,6 +237,26 @@ class Voxelizer:
             "vox_run",
         )
         return out
+
+    def run_noalloc(self, out, stream=None, stats=True):
+        """vox_run_noalloc: run() on the 4 MiB workspace built into libvox.so instead of a torch tensor.
+
+        For code that is handed its input and output tensors but may not allocate device memory itself: a plug-in
+        in an application whose pool owns the whole GPU, a loop that cannot afford the device-wide sync of an
+        allocation, a process in which another thread is capturing a graph in global mode.  `out` is therefore
+        required (nothing is allocated here either).  Jobs whose workspace_bytes exceed NOALLOC_SCRATCH_BYTES raise
+        VoxError(-3) before any GPU work.  All calls on a device share the one built-in array: keep them ordered on
+        the GPU (one stream, or events), overlapping calls race.  The first call on a device also looks up the
+        array's address; make it before any stream capture.  stats=True waits for the stream and returns the
+        vox_status dict, raising VoxError(-3) if pairs were dropped; stats=False only enqueues and returns None."""
+        torch = _torch_cuda()
+        assert out.is_cuda and out.is_contiguous() and out.numel() == self.grid_words
+        st = (ctypes.c_int64 * 4)() if stats else None
+        self._ck(self._lib.vox_run_noalloc(self._ctx, _stream_ptr(torch, stream), ctypes.c_void_p(out.data_ptr()), st),
+                 "vox_run_noalloc")
+        if st is None:
+            return None
+        return dict(pairs=int(st[0]), culled=int(st[1]), large_pairs=int(st[2]), nonempty_tiles=int(st[3]))
 
     def capture(self, out, steps=1, stream=None):
         """CUDA graph of `steps` vox_run calls into `out` (vox_run only enqueues: no sync, no allocation, so it can be

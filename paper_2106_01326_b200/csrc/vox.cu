@@ -14,6 +14,7 @@
 #include "../../include/vox.h"
 
 #include <cuda_runtime.h>
+#include <pthread.h>
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
@@ -1850,6 +1851,73 @@ extern "C" int vox_status(vox_ctx* ctx, void* cuda_stream, const void* d_workspa
         stats_out[3] = h[H_NONEMPTY];
     }
     return h[H_OVERFLOW] ? VOX_EWORKSPACE : VOX_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// vox_run_noalloc: the hot path on a workspace the library itself carries (include/vox.h)
+// ------------------------------------------------------------------------------------------
+// For callers that cannot obtain device memory at all (everything is owned by the host application's pool), must not
+// trigger the device-wide synchronisation an allocation implies, or share the process with a global-mode graph
+// capture in which cudaMalloc is an error.  The workspace is this array: part of the library's image on every
+// device that loads it, never freed.  On the HOST side the name g_noalloc_scratch is only a handle for the runtime
+// (a host shadow of the symbol), NOT a device address: handing it to a kernel would fault, or on a machine where the
+// GPU can reach host memory quietly scribble over the wrong bytes.  The device address comes from
+// cudaGetSymbolAddress, asked once per device with that device current, and is what the kernels get.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[VOX_NOALLOC_SCRATCH_BYTES];
+enum { NOALLOC_MAX_DEVICES = 64 };
+static void* g_noalloc_addr[NOALLOC_MAX_DEVICES];  // per device: address of the array there, NULL = not asked yet
+static pthread_mutex_t g_noalloc_lock = PTHREAD_MUTEX_INITIALIZER;
+
+// First call on a device: look the array's address up (this is also what makes the runtime load the library's
+// device image there, so it belongs before any stream capture).  Later calls: a table read.
+static int noalloc_scratch(vox_ctx* ctx, char** out) {
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) {
+        snprintf(ctx->err, sizeof(ctx->err), "vox_run_noalloc: device ordinal %d is beyond the %d this build keeps an address for",
+                 dev, (int)NOALLOC_MAX_DEVICES);
+        return VOX_ERANGE;
+    }
+    pthread_mutex_lock(&g_noalloc_lock);
+    void* a = g_noalloc_addr[dev];
+    cudaError_t e = cudaSuccess;
+    if (!a) {
+        e = cudaGetSymbolAddress(&a, g_noalloc_scratch);
+        if (e == cudaSuccess && a) g_noalloc_addr[dev] = a;
+    }
+    pthread_mutex_unlock(&g_noalloc_lock);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaGetSymbolAddress(g_noalloc_scratch)");
+    if (!a) {
+        snprintf(ctx->err, sizeof(ctx->err), "vox_run_noalloc: the runtime returned no address for the built-in scratch");
+        return VOX_ECUDA;
+    }
+    *out = (char*)a;
+    return VOX_OK;
+}
+
+extern "C" int vox_run_noalloc(vox_ctx* ctx, void* cuda_stream, uint32_t* d_bits_out, int64_t stats_out[4]) {
+    if (!ctx || !d_bits_out) return VOX_EINVAL;
+    if (!ctx->have_tets) return VOX_ESTATE;
+    // the size test comes first and touches no CUDA call: an oversized job is refused even where there is no device
+    const size_t need = vox_workspace_bytes(ctx);
+    if (need > (size_t)VOX_NOALLOC_SCRATCH_BYTES) {
+        snprintf(ctx->err, sizeof(ctx->err),
+                 "vox_run_noalloc: this mesh and grid need a %zu-byte workspace, the built-in scratch has %u "
+                 "(VOX_NOALLOC_SCRATCH_BYTES); use vox_run with a workspace of your own",
+                 need, (unsigned)VOX_NOALLOC_SCRATCH_BYTES);
+        return VOX_EWORKSPACE;
+    }
+    char* scratch = NULL;
+    int rc = noalloc_scratch(ctx, &scratch);
+    if (rc) return rc;
+    // The array still holds whatever the previous call (of any context) left.  run_impl starts by clearing the header,
+    // the slab bounds and the tile counters on the stream (one cudaMemsetAsync, no allocation); the cursors, the range
+    // array and the pair list are fully rewritten by K2 / K1 / K3 before they are read, so nothing else needs zeroing.
+    // The whole array is handed over: the pair list gets all the room behind the fixed part.
+    ctx->sparse = SparseOut{NULL, NULL, 0};
+    rc = run_impl(ctx, cuda_stream, scratch, (size_t)VOX_NOALLOC_SCRATCH_BYTES, d_bits_out);
+    if (rc || !stats_out) return rc;
+    return vox_status(ctx, cuda_stream, scratch, stats_out);  // waits for the stream; VOX_EWORKSPACE if pairs were dropped
 }
 
 extern "C" int vox_validate(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t ws_bytes) {
