@@ -98,6 +98,31 @@ def reduce_over_ranks(dist, ms, samples, tets, device):
     return float(t[0]), float(w[0]), float(w[1])
 
 
+def workload_config(m, input_kind, samples, stride, grid_words):
+    """The `config` object of the JSON line: what identifies the workload, and nothing about how an arm maps it to
+    hardware, so that the CUDA arm and --impl reference print the same keys (and, when the oracle runs the whole
+    workload per step, the same values).  Arm-specific facts (pairs, tile) sit under `binning` in the CUDA line."""
+    mb = (16 * m.T + 12 * m.V + 4 * grid_words) / 1e6
+    return {"workload": m.name, "input": input_kind, "tets": m.T, "verts": m.V, "grid": list(m.grid), "batch": m.batch,
+            "candidate_samples": int(samples), "bounded_sample_stride": int(stride),
+            "l2": f"no flush between steps; one step streams {mb:.0f} MB of tets+verts+grid "
+                  f"({'>' if mb > 126 else '<='} 126 MB L2)",
+            "multi_gpu": "replicas only (seed + rank), no collective"}
+
+
+def kernel_source_sha256():
+    """sha256 over the CUDA sources the library is built from (every file under csrc/, by name): ties a committed ncu
+    capture (profiles/traffic.csv, column capture_sha256) to the code being timed."""
+    import hashlib
+
+    d = os.path.join(ROOT, "paper_2106_01326_b200", "csrc")
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh", ".h")):
+            h.update(name.encode() + b"\0" + open(os.path.join(d, name), "rb").read())
+    return h.hexdigest()
+
+
 def ncu_traffic(workload, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, from the
     committed ncu --set full capture (profiles/traffic.csv names the capture); None if absent."""
@@ -114,6 +139,7 @@ def ncu_traffic(workload, kernel):
                                    "thread_inst_per_warp_inst": float(f[8]) if len(f) >= 9 else None,
                                    "shared_wavefronts": float(f[9]) if len(f) >= 10 else None,
                                    "shared_bank_conflicts": float(f[10]) if len(f) >= 11 else None}
+                best["capture_sha256"] = f[11] if len(f) >= 12 else None
         return best
     except OSError:
         return None
@@ -276,8 +302,7 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tsum / max(1, args.steps),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
         "data": "synthetic",
-        "config": {"workload": m.name, "tets": m.T, "verts": m.V, "grid": list(m.grid),
-                   "candidate_samples_full": total, "bounded_sample_stride": stride},
+        "config": workload_config(m, "tets", total, stride, m.batch * m.grid[2] * m.grid[1] * (m.grid[0] // 32)),
         "mtets_per_s": (-(-m.T // stride)) * args.steps / tsum / 1e6,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
                          "sample": info["sample"]},
@@ -581,23 +606,37 @@ def run_b200(args):
         # K4 time measured live in this run, against (i) the in-run mixed alu+fma probe and (ii) the issue slots
         executed = None
         ncu = (tr or {}).get("ncu")
-        if ncu and ncu.get("thread_inst_per_warp_inst"):
+        # the capture must belong to the code being timed: profiles/traffic.csv carries the sha256 of csrc/ at capture
+        # time; any difference (or no capture of this workload at all) nulls every figure derived from it
+        src_sha = kernel_source_sha256()
+        stale = None
+        if not ncu:
+            stale = "no committed ncu capture of this workload"
+        elif (tr or {}).get("capture_sha256") != src_sha:
+            stale = "stale capture: profiles/traffic.csv was taken from other kernel sources than the ones timed"
+        if ncu and not stale and ncu.get("thread_inst_per_warp_inst"):
             tinst = ncu["warp_inst_executed"] * ncu["thread_inst_per_warp_inst"]
             issue_peak = 148 * 4 * sm_max * 1e6  # warp instructions per second: one per cycle per SM sub-partition
             executed = {
                 "thread_inst_per_launch": tinst, "warp_inst_per_launch": ncu["warp_inst_executed"],
                 "source": (tr or {}).get("source"),
-                "achieved_tinst_per_s": tinst / (k4 * 1e-3) / 1e12,
-                "frac_mixed": (tinst / (k4 * 1e-3) / 1e12 / probe["mixed"]) if probe.get("mixed") else None,
+                "achieved_winst_per_s": ncu["warp_inst_executed"] / (k4 * 1e-3) / 1e9,
+                "issue_peak_winst_per_s": issue_peak / 1e9,
                 "frac_issue": ncu["warp_inst_executed"] / (k4 * 1e-3) / issue_peak,
                 "issue_active_pct_ncu": ncu["issue_active_pct"],
-                "unit": "T thread-instructions/s; fractions of the in-run mixed-pipe probe and of 148 x 4 issue slots x clocks.max.sm",
+                # secondary: ALL thread instructions (LDS/ATOMS/branches included) over the alu+fma-only probe: numerator
+                # and denominator are different populations, so this over-states pipe use; kept for continuity
+                "achieved_tinst_per_s": tinst / (k4 * 1e-3) / 1e12,
+                "frac_mixed_probe_all_inst": (tinst / (k4 * 1e-3) / 1e12 / probe["mixed"]) if probe.get("mixed") else None,
+                "unit": "G warp-instructions/s against 148 SMs x 4 issue slots x clocks.max.sm",
             }
-        # The fraction that BOUNDS the kernel: thread instructions it executes per second (ncu count of the committed
-        # capture of this code x lanes per instruction, over the K4 time measured live) against the integer
-        # instruction rate the SMs sustain, measured in this run by the mixed alu+fma probe.  The frozen 11/150 model
-        # of SURVEY.md 8(d) is what a per-sample incremental test would execute; the row-span kernel executes far
-        # less, so the model figure is an EFFECTIVE one (> 1) and is reported under its own name.
+        # The fraction that BOUNDS the kernel is the share of the SMs' issue slots it fills: warp instructions per
+        # launch (ncu smsp__inst_executed.sum of the committed capture of THIS code, guarded by the source hash) over
+        # the K4 time measured live, against one warp instruction per cycle per SM sub-partition.  Numerator and
+        # denominator count the same thing (every issued instruction), and ncu's own smsp__issue_active of the same
+        # capture is printed beside it.  The frozen 11/150 model of SURVEY.md 8(d) is what a per-sample incremental
+        # test would execute; the row-span kernel executes far less, so that figure is an EFFECTIVE one (> 1) and is
+        # reported under its own name.
         effective = {
             "achieved": achieved, "peak": peak_alu, "unit": "Tops/s (INT32, modelled)", "frac": achieved / peak_alu,
             "model": f"{OPS_PER_SAMPLE:g} ops/candidate sample + {OPS_PER_PAIR:g} ops/(tet,tile) pair", "ops_per_launch": ops,
@@ -607,18 +646,23 @@ def run_b200(args):
         }
         roofline = {
             "bound": "alu", "kernel": "k4_flat",
-            "achieved": (executed or {}).get("achieved_tinst_per_s"), "peak": probe.get("mixed"),
-            "unit": "T thread-instructions/s (integer alu + fma pipes)",
-            "frac": (executed or {}).get("frac_mixed"),
-            "peak_source": "measured in this run: vox_probe_int32 kind 2 (dependent-free 1:1 LOP3/IMAD stream on all SMs); "
-                           "nominal 148 SMs x 128 lanes x clocks.max.sm = %.1f" % (148 * 128 * sm_max * 1e6 / 1e12),
+            "achieved": (executed or {}).get("achieved_winst_per_s"), "peak": 148 * 4 * sm_max * 1e6 / 1e9,
+            "unit": "G warp-instructions/s (issue slots: the integer alu/fma/lsu pipes all drain through them)",
+            "frac": (executed or {}).get("frac_issue"),
+            "reason": stale,
+            "peak_source": "derived: 148 SMs x 4 sub-partitions x 1 warp instruction per cycle x clocks.max.sm "
+                           "(DESIGN.md Roofline); in-run pipe probes under peak_probe_tops",
             "frac_issue": (executed or {}).get("frac_issue"),
-            "traffic": (tr or {}).get("bytes"), "traffic_source": (tr or {}).get("source"), "ncu": ncu,
+            "issue_active_pct_ncu": (ncu or {}).get("issue_active_pct") if not stale else None,
+            "capture_sha256": (tr or {}).get("capture_sha256"), "source_sha256": src_sha,
+            "traffic": (tr or {}).get("bytes") if not stale else None, "traffic_source": (tr or {}).get("source"),
+            "ncu": ncu if not stale else None,
             "executed": executed,
-            "note": "achieved = thread instructions per K4 launch (profiles/traffic.csv: ncu smsp__inst_executed.sum x "
-                    "thread_inst_per_inst of the committed capture of this code) / K4 time measured live; frac_issue = warp "
-                    "instructions / time / (148 x 4 issue slots x clocks.max.sm).  null when no capture of this workload "
-                    "is committed.  The SURVEY 8(d) model figure is under effective_vs_bruteforce_model.",
+            "note": "achieved = warp instructions per K4 launch (profiles/traffic.csv: ncu smsp__inst_executed.sum of the "
+                    "committed capture, valid only while capture_sha256 == source_sha256) / K4 time measured live with CUDA "
+                    "events on the launching stream.  frac, traffic and ncu are null (see reason) when the capture is "
+                    "missing or was taken from other sources.  The SURVEY 8(d) model figure is under "
+                    "effective_vs_bruteforce_model.",
             "effective_vs_bruteforce_model": effective,
             "kernel_ms": k4,
             "peak_probe_tops": probe,
@@ -679,13 +723,10 @@ def run_b200(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": tmax / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "int32/int64 (exact integer)", "data": "synthetic",
-            "config": {"workload": m.name, "input": args.input + (f" (variant {args.variant})" if args.input == "lattice" else ""),
-                       "tets": m.T, "verts": m.V, "grid": list(m.grid), "batch": m.batch,
-                       "candidate_samples": samples, "pairs": pairs,
-                       "tile": [32, vz.tile_shape["ty"], vz.tile_shape["tz"]],
-                       "l2": "no flush: one step streams tets+verts+pair list+grid = "
-                             f"{(16 * m.T + 12 * m.V + 8 * m.T + 4 * pairs * 2 + 4 * vz.grid_words) / 1e6:.0f} MB > 126 MB L2",
-                       "multi_gpu": "replicas only (seed + rank), no collective"},
+            "config": workload_config(m, args.input + (f" (variant {args.variant})" if args.input == "lattice" else ""),
+                                      samples, 1, vz.grid_words),
+            "binning": {"pairs": pairs, "tile": [32, vz.tile_shape["ty"], vz.tile_shape["tz"]],
+                        "step_bytes_incl_ranges_and_pair_list": 16 * m.T + 12 * m.V + 8 * m.T + 4 * pairs * 2 + 4 * vz.grid_words},
             "mtets_per_s": tsum * args.steps / sec / 1e6,
             "gvoxels_per_s": world * m.batch * nx * ny * nz * args.steps / sec / 1e9,
             "kernel_ms": shares, "status": st, "popcount": popcount,

@@ -88,3 +88,22 @@ def test_reference_arm_line_on_small_workload():
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["value"] == line["value"]
     assert line["higher_is_better"] is True and line["steps"] == 2 and line["warmup"] == 1
+
+
+def test_both_arms_print_the_same_config_keys_and_the_capture_guard_reads_its_column():
+    """The driver compares the `config` objects of the CUDA arm and of --impl reference: one function builds both.
+    profiles/traffic.csv names, per capture, the hash of the kernel sources it was taken from; bench.py nulls
+    roofline.frac when that differs from kernel_source_sha256() of the tree being timed."""
+    import bench
+    import meshgen
+
+    m = meshgen.make_config("cfg1")
+    a = bench.workload_config(m, "tets", 1234, 1, 1024)
+    b = bench.workload_config(m, "tets", 1234, 1, 1024)
+    assert a == b and a["workload"] == m.name and a["bounded_sample_stride"] == 1 and "l2" in a
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert src.count('"config": workload_config(') == 2  # both arms, nothing hand-built beside it
+    sha = bench.kernel_source_sha256()
+    assert len(sha) == 64 and sha == bench.kernel_source_sha256()
+    row = bench.ncu_traffic("cfg4", "k4_flat")
+    assert row and len(row["capture_sha256"]) == 64
