@@ -50,7 +50,7 @@ def _args():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--input", default="tets", choices=["tets", "lattice"],
                     help="lattice: the timed steps take the mesh as lattice vertices + keep mask (vox_lattice; "
-                         "--variant 0 = fused path, 1 = through the binning passes) instead of a tet array")
+                         "--variant 0 = the library's choice, 1 = through the binning passes, 2 = fused path) instead of a tet array")
     ap.add_argument("--tile", type=int, nargs=2, default=None)
     return ap.parse_args()
 
@@ -484,9 +484,10 @@ def run_b200(args):
                 d_keep = hk.cuda()
                 e2e_lattice = {"unit": UNIT, "h2d_bytes_per_step": hv.numel() * 4 + hk.numel(), "cells": list(cells),
                                "api": f"vox_pipe_submit_lattice/vox_pipe_wait, depth {depth}",
-                               "paths": "fused = vox_lattice's default (K0 slabs + K4 enumerating its candidate cells, no "
-                                        "K1-K3, no pair list); binned = vox_set_variant(1), the same input through K1-K3"}
-                for path, lvar in (("fused", 0), ("binned", 1)):
+                               "paths": "binned = the implied tets through K1-K3 (vox_lattice's default for ordinary cells); fused = "
+                                        "vox_set_variant(2): K0 slabs + K4 enumerating its candidate cells, no K1-K3, no "
+                                        "pair list (the default's own choice only for giant cells)"}
+                for path, lvar in (("fused", 2), ("binned", 1)):
                     # device step of this path on resident inputs (its own tile: the implicit tet count picks it);
                     # the plan gives the binned path's exact pair count (outside the timing)
                     vzl = pkg.Voxelizer(m.grid, m.extent, m.batch, tile=args.tile, variant=lvar)
@@ -600,7 +601,7 @@ def run_b200(args):
         hbm_peak = peaks.get("hbm_gbs", 6650.0)
         min_bytes = 16.0 * m.T + 12.0 * m.V + 4.0 * vz.grid_words
         k4_bytes = 4.0 * vz.grid_words + pairs * (4.0 + 16.0 + 48.0)  # grid + per pair: id, tet, 4 verts
-        tr = ncu_traffic(args.workload + ("_lattice" if args.input == "lattice" and args.variant == 0 else ""), "k4_flat")
+        tr = ncu_traffic(args.workload + ("_lattice" if vz.path == "lattice_fused" else ""), "k4_flat")
         # what the kernel EXECUTES (as opposed to the frozen model of what a brute-force incremental test would):
         # thread instructions per launch from the committed ncu capture of this code (profiles/traffic.csv) over the
         # K4 time measured live in this run, against (i) the in-run mixed alu+fma probe and (ii) the issue slots
@@ -725,6 +726,7 @@ def run_b200(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "int32/int64 (exact integer)", "data": "synthetic",
             "config": workload_config(m, args.input + (f" (variant {args.variant})" if args.input == "lattice" else ""),
                                       samples, 1, vz.grid_words),
+            "path": vz.path,
             "binning": {"pairs": pairs, "tile": [32, vz.tile_shape["ty"], vz.tile_shape["tz"]],
                         "step_bytes_incl_ranges_and_pair_list": 16 * m.T + 12 * m.V + 8 * m.T + 4 * pairs * 2 + 4 * vz.grid_words},
             "mtets_per_s": tsum * args.steps / sec / 1e6,

@@ -69,11 +69,17 @@ void vox_destroy(vox_ctx* ctx);
  * result of vox_run does not depend on the tile; vox_tile_shape reports it. */
 int vox_set_tile(vox_ctx* ctx, int ty, int tz);
 
-/* Path variant for A/B runs and cross-checks, 0 = default.  Result-neutral by contract.
- *   1: lattice input (vox_lattice) goes through the binning passes K1-K3 like a tet array instead of the fused
- *      lattice path; no effect on explicit tets.
- * Any other value is refused with VOX_EINVAL (never silently ignored). */
+/* Path variant, 0 = default.  Result-neutral by contract; only lattice input (vox_lattice) has a choice to make:
+ *   0: the library picks: the binning passes K1-K3 (the faster device step on every measured workload of ordinary
+ *      cells), the fused lattice path only when the mean cell is at least 64^3 voxels (giant cells);
+ *   1: always the binning passes;
+ *   2: the fused lattice path whenever the lattice is within its limits (see vox_lattice) -- the small-workspace
+ *      variant: no range array, no pair list.
+ * Any other value is refused with VOX_EINVAL (never silently ignored).  vox_path reports the path the next vox_run
+ * takes: 0 = tet array through the binning passes, 1 = lattice input through the binning passes, 2 = lattice input
+ * on the fused path (VOX_ESTATE before vox_tets / vox_lattice). */
 int vox_set_variant(vox_ctx* ctx, int variant);
+int vox_path(const vox_ctx* ctx);
 
 /* Borrow the mesh.  d_verts int32[V][3] with coordinates in [0, extent];
  * d_tets int32[T][4], indices global into d_verts; d_tet_offsets int64[batch+1]
@@ -91,14 +97,16 @@ int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const int32_t* d_t
  * (xyz, xzy, yxz, yzx, zxy, zyx); bit q of d_keep[c] says whether tet q is present.  Equivalent to vox_tets with
  * the 6*cx*cy*cz tets written out (absent ones dropped).  With batch > 1 every mesh has the same lattice dims:
  * mesh m's vertices and keep bytes are the m-th block of d_verts / d_keep.
- * vox_run on lattice input takes the FUSED path: a pass over the vertices (K0) records, per axis and vertex plane
+ * vox_run on lattice input takes the binning passes over the implied tets by default (vox_set_variant above).  The
+ * FUSED path (variant 2, or the default's own choice for giant cells): a pass over the vertices (K0) records, per axis and vertex plane
  * of the lattice, the coordinate range of the plane; each tile then finds the index box of the cells that can
  * reach it from those ranges and its own coordinates, enumerates their present tets and voxelizes them -- no
  * per-tet bbox search, no pair list, no K1/K2/K3 (the exact per-tet box inside the tile kernel keeps the result
  * the definition's).  Its workspace is the header, 8*(cx+cy+cz+3) bytes per mesh and a 16-byte copy of every vertex
- * (vox_workspace_bytes);
+ * (vox_workspace_bytes: on this path it is SMALLER than vox_workspace_fixed_bytes, which is what the optional vox_plan
+ * needs -- the fused path has no pair list to size, so plan only if the pair count itself is wanted);
  * vox_status then reports culled = 0 (slivers and degenerate tets are skipped per tile, not counted per tet).
- * Lattices beyond 4096 cells per axis, 2^28 vertices or 65535 meshes, and vox_set_variant(ctx, 1), take the binning passes
+ * Lattices beyond 4096 cells per axis, 2^28 vertices or 65535 meshes take the binning passes whatever the variant
  * (vox_status then counts only present tets as culled).  vox_plan always runs the binning count. */
 int vox_lattice(vox_ctx* ctx, const int32_t* d_verts, int cx, int cy, int cz, const uint8_t* d_keep);
 
@@ -280,7 +288,8 @@ const char* vox_pipe_last_error(const vox_pipe* pipe);
  * 0,1,2,... from the enable call.  vox_timing_read(ctx, run, ms) returns the
  * durations {K1 incl. memset, K2, K3, K4, whole run} in milliseconds of a run that
  * has COMPLETED (the caller synchronises) and is still in the ring, else VOX_ESTATE.
- * slots == 0 disables and frees. */
+ * A vox_run enqueued on a stream that is being captured into a CUDA graph records no events
+ * and takes no run number.  slots == 0 disables and frees. */
 int vox_timing_enable(vox_ctx* ctx, int slots);
 int vox_timing_read(vox_ctx* ctx, int run, float ms_out[5]);
 

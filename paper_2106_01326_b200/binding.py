@@ -19,7 +19,7 @@ EXPORTS = [
     "vox_pipe_bind", "vox_pipe_submit", "vox_pipe_wait", "vox_pipe_last_error",
     "vox_tile_shape", "vox_run_sparse", "vox_sparse_status", "vox_pipe_submit_sparse", "vox_pipe_tile_shape",
     "vox_pipe_reserve_pairs", "vox_occupancy", "vox_lattice", "vox_pipe_submit_lattice", "vox_kernel_launches",
-    "vox_debug_check_status", "vox_run_noalloc",
+    "vox_debug_check_status", "vox_run_noalloc", "vox_path",
 ]
 
 
@@ -89,6 +89,7 @@ def load_library():
         "vox_kernel_launches": (ctypes.c_uint64, []),
         "vox_debug_check_status": (i32, [ctypes.POINTER(ctypes.c_uint32)]),
         "vox_run_noalloc": (i32, [vp, vp, vp, ctypes.POINTER(i64)]),
+        "vox_path": (i32, [vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -142,12 +143,14 @@ class Voxelizer:
         self._keep = None
         self._ws = None
         self._out = None
+        self._generation = 0  # bumped whenever the mesh or the workspace is re-bound (CapturedStep checks it)
 
     def _ck(self, rc, where):
         if rc:
             raise VoxError(rc, where, self._lib.vox_last_error(self._ctx).decode())
 
     def close(self):
+        self._generation += 1
         if self._ctx:
             self._lib.vox_destroy(self._ctx)
             self._ctx = ctypes.c_void_p()
@@ -187,6 +190,7 @@ class Voxelizer:
             "vox_tets",
         )
         self._keep = (verts, tets, tet_offsets)
+        self._generation += 1
         self.T, self.V = T, V
 
     def set_lattice(self, verts, cells, keep):
@@ -200,12 +204,14 @@ class Voxelizer:
         self._ck(self._lib.vox_lattice(self._ctx, ctypes.c_void_p(verts.data_ptr()), cx, cy, cz,
                                        ctypes.c_void_p(keep.data_ptr())), "vox_lattice")
         self._keep = (verts, keep)
+        self._generation += 1
         self.T, self.V = self.batch * 6 * cx * cy * cz, self.batch * (cx + 1) * (cy + 1) * (cz + 1)
 
     def alloc_workspace(self, nbytes=None):
         torch = _torch_cuda()
         n = int(nbytes if nbytes is not None else self.workspace_bytes)
         self._ws = torch.empty(max(n, 256), dtype=torch.uint8, device="cuda")
+        self._generation += 1
         return self._ws
 
     def plan(self, stream=None):
@@ -260,9 +266,12 @@ class Voxelizer:
 
     def capture(self, out, steps=1, stream=None):
         """CUDA graph of `steps` vox_run calls into `out` (vox_run only enqueues: no sync, no allocation, so it can be
-        stream-captured).  Returns the torch.cuda.CUDAGraph; replay() re-runs the step(s) on the mesh, workspace and
-        output bound now.  Worth ~6-8 us per step: it removes the launch gaps between the memset and the four kernels,
-        which is a sixth of a step on the smallest configs and nothing on the large ones."""
+        stream-captured).  Returns a CapturedStep; replay() re-runs the step(s) on the mesh, workspace and output
+        bound at capture time and refuses (RuntimeError) once set_tets / set_lattice / alloc_workspace / plan / close
+        has re-bound any of them, because the graph has the old pointers and sizes baked in.  Runs inside the capture
+        record no timing events (vox_timing_*).  Worth ~6-8 us per step: it removes the launch gaps between the memset
+        and the four kernels, which is a sixth of a step on the smallest configs and nothing on the large ones
+        (DESIGN.md 8)."""
         torch = _torch_cuda()
         if self._ws is None:
             self.alloc_workspace()
@@ -274,7 +283,15 @@ class Voxelizer:
             with torch.cuda.graph(g, stream=stream):
                 for _ in range(int(steps)):
                     self.run(out, stream)
-        return g
+        return CapturedStep(self, g, out)
+
+    @property
+    def path(self):
+        """vox_path: 'tets' (tet array through K1-K4), 'lattice_binned' or 'lattice_fused' -- what the next run() takes."""
+        rc = self._lib.vox_path(self._ctx)
+        if rc < 0:
+            raise VoxError(rc, "vox_path")
+        return ("tets", "lattice_binned", "lattice_fused")[rc]
 
     @property
     def tile_shape(self):
@@ -361,6 +378,22 @@ class Voxelizer:
             "vox_run_host",
         )
         return h_out
+
+
+class CapturedStep:
+    """A CUDA graph of vox_run steps (Voxelizer.capture).  The graph holds the mesh pointers, the workspace pointer
+    and capacity, the tile and the output pointer as they were at capture time; replay() checks that the Voxelizer
+    has not re-bound any of them since."""
+
+    def __init__(self, vz, graph, out):
+        self._vz, self.graph, self._out = vz, graph, out  # (keeps the output tensor alive)
+        self._generation = vz._generation
+
+    def replay(self):
+        if self._vz._generation != self._generation:
+            raise RuntimeError("CapturedStep.replay: the Voxelizer's mesh or workspace was re-bound (set_tets / "
+                               "set_lattice / alloc_workspace / plan / close) after the capture; capture again")
+        self.graph.replay()
 
 
 class Pipe:

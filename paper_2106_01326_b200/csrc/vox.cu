@@ -1597,21 +1597,37 @@ extern "C" int vox_set_tile(vox_ctx* ctx, int ty, int tz) {
     return VOX_OK;
 }
 
-// lattice input takes the fused path (K0 + K4, no binning) unless variant 1 asks for the binned one or the lattice
-// is beyond what k0_slabs / the candidate queue were sized for
+// Which path lattice input takes.  The binning passes (K1-K3 over the implied tets, then K4 on the pair lists) are the
+// default: measured on every workload of profiles/r02_workloads.md they are the faster device step (cfg4 1.54 vs 1.72
+// ms, cfg3 0.69 vs 0.89, cfg5 0.56 vs 0.84) except where cells are giants of many tiles each (S1: 0.245 vs 0.222), which
+// is where the default picks the fused path (K0 + K4 enumerating its own candidates) by itself.  vox_set_variant(2)
+// asks for the fused path regardless (its merit is the small workspace: no range array, no pair list), variant 1
+// forbids it.  Lattices beyond what k0_slabs / the candidate queue were sized for always take the binning passes.
+static bool fused_possible(const Params& p) {
+    return p.lcx > 0 && p.lcx <= 4096 && p.lcy <= 4096 && p.lcz <= 4096 && p.V < (1ll << 28) &&
+           p.batch <= 65535;  // (k0_slabs: shared-memory z table, gridDim.z = batch; queue entries are v0 << 3 | q)
+}
 static bool lattice_fused(const vox_ctx* ctx) {
     const Params& p = ctx->p;
-    return p.lcx > 0 && ctx->variant == 0 && p.lcx <= 4096 && p.lcy <= 4096 && p.lcz <= 4096 && p.V < (1ll << 28) &&
-           p.batch <= 65535;  // (k0_slabs: shared-memory z table, gridDim.z = batch; queue entries are v0 << 3 | q)
+    if (!fused_possible(p) || ctx->variant == 1) return false;
+    if (ctx->variant == 2) return true;
+    // default: only for giant cells -- a mean cell of at least 64^3 voxels (two 32-voxel tiles per axis or more)
+    return (i64)p.nx * p.ny * p.nz >= 262144ll * p.lcx * p.lcy * p.lcz;
 }
 
 extern "C" int vox_set_variant(vox_ctx* ctx, int variant) {
-    // 0: default.  1: lattice input goes through the binning passes K1-K3 like a tet array (cross-check of the
-    // fused lattice path; no effect on explicit tets)
-    if (!ctx || (variant != 0 && variant != 1)) return VOX_EINVAL;
+    // 0: default.  1: lattice input always goes through the binning passes K1-K3 like a tet array.  2: lattice input
+    // takes the fused path whenever the lattice is within its limits.  No effect on explicit tets.
+    if (!ctx || variant < 0 || variant > 2) return VOX_EINVAL;
     ctx->variant = variant;
     ctx->p.fused = lattice_fused(ctx) ? 1 : 0;
     return VOX_OK;
+}
+
+extern "C" int vox_path(const vox_ctx* ctx) {
+    if (!ctx) return VOX_EINVAL;
+    if (!ctx->have_tets) return VOX_ESTATE;
+    return ctx->p.lcx == 0 ? 0 : (lattice_fused(ctx) ? 2 : 1);
 }
 
 extern "C" int vox_tets(vox_ctx* ctx, const int32_t* d_verts, int64_t V, const int32_t* d_tets, int64_t T,
@@ -1772,7 +1788,12 @@ static int run_impl(vox_ctx* ctx, void* cuda_stream, void* d_workspace, size_t w
     WsLayout L = ws_layout(p);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char* ws = (char*)d_workspace;
-    cudaEvent_t* ev = ctx->tm_ev ? ctx->tm_ev + (size_t)(ctx->tm_next % ctx->tm_slots) * TM_EV : NULL;
+    // per-kernel timing events are not recorded into a stream capture: a captured record would be replayed with every
+    // graph launch and vox_timing_read would see events that never completed outside the graph
+    cudaStreamCaptureStatus cap_status = cudaStreamCaptureStatusNone;
+    if (ctx->tm_ev) CK(cudaStreamIsCapturing(st, &cap_status));
+    cudaEvent_t* ev = (ctx->tm_ev && cap_status == cudaStreamCaptureStatusNone)
+                          ? ctx->tm_ev + (size_t)(ctx->tm_next % ctx->tm_slots) * TM_EV : NULL;
     if (lattice_fused(ctx)) {  // K0 (vertex-plane slabs) + K4 enumerating its own candidates
         if (ws_bytes < L.counts + (size_t)p.V * 16) return VOX_EWORKSPACE;
         u32* hdr = (u32*)(ws + L.hdr);
@@ -2109,7 +2130,14 @@ static void pipe_layout(vox_pipe* q) {
     vox_ctx tmp = *q->slot[0].ctx;
     tmp.p.T = q->maxT;
     tmp.pairs_planned = q->reserve_pairs > 0 ? q->reserve_pairs : -1;
-    q->A = arena_layout(&tmp, q->maxV, q->maxT, vox_workspace_bytes(&tmp));
+    // the workspace of a slice must serve whichever path a submitted mesh takes: the binned layout (sized here from
+    // max_T and the pair reservation) or, for lattice input on the fused path, header + vertex-plane slabs + the 16-byte
+    // vertex copy.  Lattice dims are not known yet; (cx+1) + (cy+1) + (cz+1) <= V + 2 per mesh bounds the slabs.
+    size_t ws = vox_workspace_bytes(&tmp);
+    const size_t fused_ws = align256(HDR_WORDS * 4) + align256(8 * ((size_t)q->maxV + 2 * (size_t)tmp.p.batch)) +
+                            align256(16 * (size_t)q->maxV);
+    if (fused_ws > ws) ws = fused_ws;
+    q->A = arena_layout(&tmp, q->maxV, q->maxT, ws);
     q->slice_bytes = align256(q->A.end);
 }
 

@@ -96,14 +96,14 @@ def test_parity_is_tile_independent(name, tile):
 
 
 def test_unknown_kernel_variant_is_refused():
-    # variants 0 (default) and 1 (binned lattice path) exist; any other must be refused, never silently ignored
+    # variants 0 (default), 1 (binned lattice path) and 2 (fused lattice path) exist; any other must be refused
     import paper_2106_01326_b200 as pkg
 
     with pytest.raises(pkg.VoxError) as ei:
         pkg.Voxelizer((32, 32, 32), variant=3)
     assert ei.value.code == -1
     with pytest.raises(pkg.VoxError):
-        pkg.Pipe((32, 32, 32), depth=1, max_V=4, max_T=1, variant=2)
+        pkg.Pipe((32, 32, 32), depth=1, max_V=4, max_T=1, variant=4)
 
 
 def test_graph_replay_of_a_step_matches_oracle():
@@ -129,6 +129,46 @@ def test_graph_replay_of_a_step_matches_oracle():
             assert_same(out.cpu().numpy().view(np.uint32), exp, f"graph replay {name}")
         assert vz.status()["pairs"] > 0
         vz.close()
+
+
+def test_graph_capture_skips_timing_events_and_refuses_a_rebound_voxelizer():
+    """With vox_timing_enable active a captured vox_run records no events and takes no run number (the events of the
+    runs outside the capture stay readable); a CapturedStep refuses to replay once the Voxelizer's workspace or mesh
+    has been re-bound, because the graph still holds the old pointers."""
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    m = CASES["cfg2"]()
+    exp = cpu_voxelize(m)
+    vz = pkg.Voxelizer(m.grid, m.extent, m.batch)
+    vz.set_tets(torch.from_numpy(m.verts).cuda(), torch.from_numpy(m.tets).cuda())
+    vz.plan()
+    vz.timing_enable(8)
+    nx, ny, nz = m.grid
+    out = torch.empty((1, nz, ny, nx // 32), dtype=torch.int32, device="cuda")
+    vz.run(out)                      # run 0
+    g = vz.capture(out, steps=2)     # its warm-up outside the capture is run 1; the two captured runs take no number
+    torch.cuda.synchronize()
+    for run in (0, 1):
+        ms = vz.timing_read(run)
+        assert ms["total"] > 0 and ms["k4"] > 0
+    with pytest.raises(pkg.VoxError) as ei:
+        vz.timing_read(2)
+    assert ei.value.code == -5
+    for _ in range(2):
+        out.fill_(-1)
+        g.replay()
+        torch.cuda.synchronize()
+        assert_same(out.cpu().numpy().view(np.uint32), exp, "graph replay with timing enabled")
+    assert vz.timing_read(1)["total"] > 0     # replays did not disturb the ring
+    vz.run(out)                                # run 2, outside any capture
+    torch.cuda.synchronize()
+    assert vz.timing_read(2)["total"] > 0
+    vz.alloc_workspace()                       # re-binds the workspace: the graph's pointer is stale
+    with pytest.raises(RuntimeError):
+        g.replay()
+    vz.close()
 
 
 def test_estimated_workspace_path():
@@ -549,7 +589,43 @@ def test_randomized_magnitudes_straddle_the_int32_limit():
         assert_same(gpu_voxelize(m, tile=tile), cpu_voxelize(m), f"magnitude seed {seed} n {n} E {Ex} tile {tile}")
         large += pkg.voxelize.last_status["large_pairs"]
         pairs += pkg.voxelize.last_status["pairs"]
-    assert 0.1 * pairs < large < 0.9 * pairs, (large, pairs)
+    print(f"straddle: large={large} span={pairs - large} pairs={pairs}")
+    # fixed seeds: explicit floors on BOTH sides of the hand-over (measured at round 3: see the printed line with -s)
+    assert large >= STRADDLE_MIN_LARGE and pairs - large >= STRADDLE_MIN_SPAN, (large, pairs)
+
+
+# measured with these seeds at round 3: 11 941 pairs on the int64 path, 5 009 on the int32 span path (of 16 950).  A change
+# that moves the hand-over may move these by a little; one that pushes either side below the floor has stopped
+# exercising that side and must say so by changing the floor.
+STRADDLE_MIN_LARGE = 10000
+STRADDLE_MIN_SPAN = 4000
+
+
+def test_single_tet_swept_across_the_int32_hand_over():
+    """One tet shape grown in 2 % steps from 2^12 to 2^15.4 lattice units on a 256^3 grid of extent 2^20 (pitch 4096):
+    the int32 span record holds it at the small end (plane values ~ d^3 / g below 2^31) and cannot at the large end, so
+    the sweep crosses the hand-over bound with neighbours 2 % apart on either side of it -- every grid against the
+    oracle, on two tile shapes, and both ends must be on the side they belong to."""
+    import paper_2106_01326_b200 as pkg
+
+    Ex, n = 1 << 20, 256
+    base = np.array([300000, 410000, 520000])
+    shape = np.array([[0.0, 0.0, 0.0], [1.0, 0.13, 0.21], [0.17, 0.93, 0.08], [0.22, 0.31, 0.97]])
+    for tile in ((32, 32), (8, 8)):
+        flags = []
+        for k in range(120):
+            d = 4096.0 * 1.02 ** k
+            pts = np.clip(np.rint(base + shape * d).astype(np.int64), 0, Ex)
+            m = Mesh(f"sweep{k}", pts.astype(np.int32), np.array([[0, 1, 2, 3]], dtype=np.int32), (n, n, n), (Ex,) * 3)
+            assert_same(gpu_voxelize(m, tile=tile), cpu_voxelize(m), f"sweep k={k} d={d:.0f} tile={tile}")
+            st = pkg.voxelize.last_status
+            assert st["pairs"] >= 1
+            flags.append(st["large_pairs"] / st["pairs"])
+        assert all(f == 0.0 for f in flags[:10]), (tile, flags[:10])      # small end: int32 span records only
+        assert all(f == 1.0 for f in flags[-10:]), (tile, flags[-10:])    # large end: int64 path only
+        first_large = next(i for i, f in enumerate(flags) if f > 0)
+        last_span = max(i for i, f in enumerate(flags) if f < 1)
+        assert 10 <= first_large <= last_span + 1 <= 110, (tile, first_large, last_span)
 
 
 def test_fast_setup_fit_test_is_straddled():

@@ -123,10 +123,12 @@ def _pin(a):
     return torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
 
 
+@pytest.mark.parametrize("variant", [0, 2], ids=["default", "fused"])
 @pytest.mark.parametrize("name", ["cfg4", "cfg3"])
-def test_lattice_input_full_size_device_and_pipe(name):
+def test_lattice_input_full_size_device_and_pipe(name, variant):
     """vox_lattice (device pointers) and vox_pipe_submit_lattice (host buffers), dense and sparse, on the whole of
-    cfg4 / cfg3 -- against the oracle on the tets written out, not against the tet-array GPU run."""
+    cfg4 / cfg3 -- against the oracle on the tets written out, not against the tet-array GPU run.  The default takes
+    the binning passes on these (cells of 8 and 2.7 voxels); variant 2 is the fused small-workspace path."""
     import torch
 
     import paper_2106_01326_b200 as pkg
@@ -138,9 +140,10 @@ def test_lattice_input_full_size_device_and_pipe(name):
     keep = meshgen.lattice_form(m, cells)
     assert int(np.unpackbits(keep).sum()) == m.T
     d_verts, d_keep = torch.from_numpy(m.verts).cuda(), torch.from_numpy(keep).cuda()
-    vz = pkg.Voxelizer(m.grid, m.extent, m.batch)
+    vz = pkg.Voxelizer(m.grid, m.extent, m.batch, variant=variant)
     try:
         vz.set_lattice(d_verts, cells, d_keep)
+        assert vz.path == ("lattice_fused" if variant == 2 else "lattice_binned")
         vz.plan()
         got = vz.run().cpu().numpy().view(np.uint32)
         st = vz.status()
@@ -157,7 +160,7 @@ def test_lattice_input_full_size_device_and_pipe(name):
         vz.close()
     del d_verts, d_keep
     lat_T = m.batch * 6 * cells[0] * cells[1] * cells[2]
-    pipe = pkg.Pipe(m.grid, m.extent, m.batch, depth=2, max_V=m.V, max_T=lat_T)
+    pipe = pkg.Pipe(m.grid, m.extent, m.batch, depth=2, max_V=m.V, max_T=lat_T, variant=variant)
     try:
         pts = pipe.tile_shape
         pnb = m.batch * pts["nbx"] * pts["nby"] * pts["nbz"]

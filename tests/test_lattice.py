@@ -53,10 +53,10 @@ def _cases():
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("variant", [0, 1], ids=["fused", "binned"])
+@pytest.mark.parametrize("variant", [2, 1], ids=["fused", "binned"])
 @pytest.mark.parametrize("idx", range(8))
 def test_gpu_lattice_input_matches_oracle(idx, variant):
-    """variant 0: the fused lattice path (K0 slabs + tiles enumerating their own candidate cells, no K1-K3);
+    """variant 2: the fused lattice path (K0 slabs + tiles enumerating their own candidate cells, no K1-K3);
     variant 1: the same input through the binning passes.  Both must give the oracle's grid and count the same
     (tet, tile) pairs as the tet array written out."""
     import torch
@@ -68,7 +68,8 @@ def test_gpu_lattice_input_matches_oracle(idx, variant):
     keep = meshgen.lattice_form(m, cells)
     vz = pkg.Voxelizer(m.grid, m.extent, m.batch, variant=variant)
     vz.set_lattice(torch.from_numpy(m.verts).cuda(), cells, torch.from_numpy(keep).cuda())
-    if variant == 0:    # header + slabs + the 16-byte vertex copy: no counters, no range array, no pair list
+    assert vz.path == ("lattice_fused" if variant == 2 else "lattice_binned")
+    if variant == 2:    # header + slabs + the 16-byte vertex copy: no counters, no range array, no pair list
         assert vz.workspace_bytes <= 1024 + 8 * m.batch * (sum(cells) + 3) + 16 * m.V + 768
     pairs = vz.plan()
     got = vz.run().cpu().numpy().view(np.uint32)
@@ -89,7 +90,52 @@ def test_gpu_lattice_input_matches_oracle(idx, variant):
 
 
 @pytest.mark.gpu
-def test_gpu_lattice_through_the_pipe_dense_and_sparse():
+def test_gpu_default_path_of_lattice_input_and_launch_counts():
+    """The default (variant 0) sends lattice input through the binning passes and picks the fused path by itself only
+    for giant cells (mean cell >= 64^3 voxels); vox_path says which.  The launch counter (bench.py's gpu_launches)
+    rises by exactly 4 per binned run (K1, K2, K3, K4) and by 2 per fused run (K0, K4)."""
+    import torch
+
+    import paper_2106_01326_b200 as pkg
+
+    expect = {"cfg1_sphere": "lattice_binned", "cfg4_small_drop3": "lattice_binned", "giant": "lattice_fused"}
+    seen = set()
+    for name, m, cells in _cases():
+        if name not in expect or m.batch > 1:
+            continue
+        seen.add(name)
+        exp = oracle.voxelize(m.verts, m.tets, m.grid, m.extent)
+        keep = meshgen.lattice_form(m, cells)
+        dv, dk = torch.from_numpy(m.verts).cuda(), torch.from_numpy(keep).cuda()
+        for variant, path in ((0, expect[name]), (1, "lattice_binned"), (2, "lattice_fused")):
+            vz = pkg.Voxelizer(m.grid, m.extent, 1, variant=variant)
+            vz.set_lattice(dv, cells, dk)
+            assert vz.path == path, (name, variant, vz.path)
+            vz.plan()
+            out = vz.run()
+            torch.cuda.synchronize()
+            before = pkg.kernel_launches()
+            for _ in range(3):
+                vz.run(out)
+            assert pkg.kernel_launches() - before == 3 * (2 if path == "lattice_fused" else 4), (name, variant)
+            assert np.array_equal(out.cpu().numpy().view(np.uint32), exp), (name, variant)
+            vz.close()
+        # the tet array: path 'tets', 4 launches
+        vz = pkg.Voxelizer(m.grid, m.extent, 1)
+        vz.set_tets(dv, torch.from_numpy(m.tets).cuda())
+        assert vz.path == "tets"
+        vz.plan()
+        out = vz.run()
+        before = pkg.kernel_launches()
+        vz.run(out)
+        assert pkg.kernel_launches() - before == 4
+        vz.close()
+    assert seen == set(expect)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("variant", [0, 2], ids=["default", "fused"])
+def test_gpu_lattice_through_the_pipe_dense_and_sparse(variant):
     import torch
 
     import paper_2106_01326_b200 as pkg
@@ -99,7 +145,7 @@ def test_gpu_lattice_through_the_pipe_dense_and_sparse():
     exp = oracle.voxelize(m.verts, m.tets, m.grid, m.extent)
     keep = meshgen.lattice_form(m, cells)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    pipe = pkg.Pipe(m.grid, m.extent, depth=3, max_V=m.V, max_T=6 * cells[0] * cells[1] * cells[2])
+    pipe = pkg.Pipe(m.grid, m.extent, depth=3, max_V=m.V, max_T=6 * cells[0] * cells[1] * cells[2], variant=variant)
     ts = pipe.tile_shape
     nb = ts["nbx"] * ts["nby"] * ts["nbz"]
     nx, ny, nz = m.grid
@@ -165,7 +211,7 @@ def test_gpu_random_lattices_match_oracle(block):
         exp = oracle.voxelize(m.verts, m.tets, m.grid, m.extent)
         keep = meshgen.lattice_form(m, cells)
         pairs = []
-        for variant in (0, 1):
+        for variant in (2, 1):
             vz = pkg.Voxelizer(m.grid, m.extent, 1, variant=variant)
             vz.set_lattice(torch.from_numpy(m.verts).cuda(), cells, torch.from_numpy(keep).cuda())
             vz.plan()
@@ -198,7 +244,7 @@ def test_gpu_fused_lattice_with_a_huge_index_box():
     dv, dk = torch.from_numpy(m.verts).cuda(), torch.from_numpy(keep).cuda()
     pairs = {}
     for tile in ((32, 32), (8, 8)):
-        for variant in (0, 1):
+        for variant in (2, 1):
             vz = pkg.Voxelizer(m.grid, m.extent, 1, tile=tile, variant=variant)
             vz.set_lattice(dv, (C, C, C), dk)
             vz.plan()
@@ -206,4 +252,4 @@ def test_gpu_fused_lattice_with_a_huge_index_box():
             pairs[(tile, variant)] = vz.status()["pairs"]
             vz.close()
             assert np.array_equal(got, exp), f"tile {tile} variant {variant}: {(got != exp).sum()} words differ"
-        assert pairs[(tile, 0)] == pairs[(tile, 1)] > 0
+        assert pairs[(tile, 2)] == pairs[(tile, 1)] > 0
