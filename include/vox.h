@@ -310,6 +310,20 @@ uint64_t vox_kernel_launches(void);
  * check and returns 0.  Test instrumentation: compute-sanitizer is closed on this pool (profiles/r02_sanitizers.md). */
 int vox_debug_check_status(uint32_t* code_out);
 
+/* Checked build only (the normal library compiles no test kernel and returns 0): runs the integer helpers the row
+ * walk of K4 is built on over caller-supplied operand arrays, one element per thread, so that a test can compare them
+ * with exact integer division operand by operand instead of through whole meshes (a compiler mis-fold corrupted
+ * exactly this code twice).  d_a, d_b int64[n], d_out int32[n], all on the device; enqueue only.
+ *   op 0: span_bound(r = a, mx = -b, inv = recip_up(b))      the per-row bound with the fast set-up's reciprocal
+ *   op 1: span_bound(r = a, mx = -b, inv = 0xFFFFFFFF/b + 1)  the same with the general set-up's exact reciprocal
+ *         contract (4 <= b < 2^31, |a|(1 + 2^-18) + b < 2^31): a >= 0 and a/b < 2^18 -> floor(a/b); a/b >= 2^18 -> some
+ *         value >= 2^18 - 1; a < 0 -> some value <= -1
+ *   op 2: (a * div_magic(b)) >> 16 = a / b for 0 <= a < 1024, 1 <= b <= 32   (row index -> slice of the local box)
+ *   op 3: span64_bound(q0 = a, a = b) = max{x in [0,31] : q0 - b*x >= 0} or -1   (int64 large path)
+ *   op 4: recip_up(b): in [2^32/b, (2^32/b)(1 + 2^-19) + 1), never below 2^32/b
+ * Returns 1 when the kernel was enqueued, 0 in the normal build, a negative code on bad arguments. */
+int vox_debug_selftest(void* cuda_stream, int op, const int64_t* d_a, const int64_t* d_b, int64_t n, int32_t* d_out);
+
 const char* vox_strerror(int code);
 const char* vox_last_error(const vox_ctx* ctx); /* CUDA error text of the last VOX_ECUDA */
 

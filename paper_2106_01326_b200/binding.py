@@ -19,7 +19,7 @@ EXPORTS = [
     "vox_pipe_bind", "vox_pipe_submit", "vox_pipe_wait", "vox_pipe_last_error",
     "vox_tile_shape", "vox_run_sparse", "vox_sparse_status", "vox_pipe_submit_sparse", "vox_pipe_tile_shape",
     "vox_pipe_reserve_pairs", "vox_occupancy", "vox_lattice", "vox_pipe_submit_lattice", "vox_kernel_launches",
-    "vox_debug_check_status", "vox_run_noalloc", "vox_path",
+    "vox_debug_check_status", "vox_run_noalloc", "vox_path", "vox_debug_selftest",
 ]
 
 
@@ -90,6 +90,7 @@ def load_library():
         "vox_debug_check_status": (i32, [ctypes.POINTER(ctypes.c_uint32)]),
         "vox_run_noalloc": (i32, [vp, vp, vp, ctypes.POINTER(i64)]),
         "vox_path": (i32, [vp]),
+        "vox_debug_selftest": (i32, [vp, i32, vp, vp, i64, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
