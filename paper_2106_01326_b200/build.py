@@ -9,8 +9,13 @@ import subprocess
 import sys
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(_HERE, "csrc", "vox.cu")
+SRC = os.path.join(_HERE, "csrc", "vox.cu")  # the one translation unit; it includes the .cuh parts beside it
 HDR = os.path.join(os.path.dirname(_HERE), "include", "vox.h")
+
+
+def _deps():
+    d = os.path.dirname(SRC)
+    return [os.path.join(d, f) for f in sorted(os.listdir(d)) if f.endswith((".cu", ".cuh", ".h"))] + [HDR]
 LIB = os.path.join(_HERE, "libvox.so")
 
 NVCC_FLAGS = [
@@ -27,7 +32,7 @@ def build_checked(force: bool = False) -> str:
     """The same source with -DVOX_CHECKS: device-side bounds checks on every index the kernels form
     (vox_debug_check_status; tests/test_gpu_checked_build.py)."""
     if force or not os.path.exists(LIB_CHECKED) or any(
-            os.path.getmtime(f) > os.path.getmtime(LIB_CHECKED) for f in (SRC, HDR)):
+            os.path.getmtime(f) > os.path.getmtime(LIB_CHECKED) for f in _deps()):
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB_CHECKED + f".tmp{os.getpid()}"
         subprocess.check_call([nvcc] + NVCC_FLAGS + ["-DVOX_CHECKS", "-o", tmp, SRC])
@@ -39,7 +44,7 @@ def needs_build() -> bool:
     if not os.path.exists(LIB):
         return True
     m = os.path.getmtime(LIB)
-    return any(os.path.getmtime(f) > m for f in (SRC, HDR))
+    return any(os.path.getmtime(f) > m for f in _deps())
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

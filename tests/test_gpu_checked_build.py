@@ -45,7 +45,7 @@ def test_parity_subset_under_the_checked_build():
     res = json.loads(lines[-1][len("CHECKED_RESULT "):])
     assert res["lib"] == lib and res["compiled"] is True, res
     assert res["rc"] == 0, out.stdout[-3000:]
-    assert res["check"] == 0, f"device-side check {res['check']} was violated (codes: csrc/vox.cu CK_*)"
+    assert res["check"] == 0, f"device-side check {res['check']} was violated (codes: csrc/common.cuh CK_*)"
 
 
 def test_a_violated_check_is_reported():
