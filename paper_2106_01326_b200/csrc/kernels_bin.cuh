@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
     // naming the same tile (neighbouring tets mostly do) are merged into one atomic
     live = live && !handed;
     int cx = b0x, cy = b0y, cz = b0z;
-    const int lane = threadIdx.x & 31;
+    const u32 lt = (1u << (threadIdx.x & 31)) - 1u;
     for (;;) {
         const unsigned act = __ballot_sync(0xFFFFFFFFu, live);
         if (!act) break;
@@ -54,7 +54,9 @@ __global__ void __launch_bounds__(256) k1_count(Params p, uint2* __restrict__ ra
             const u32 b = ((((u32)m * p.nbz + cz) * p.nby + cy) * p.nbx) + cx;
             VOX_CHECK(b < p.NB, CK_K1_TILE);
             const unsigned peers = __match_any_sync(act, b);
-            if (lane == __ffs(peers) - 1) atomicAdd(counts + b, (u32)__popc(peers));
+            // (the group's lowest lane adds for all of it; "no peer below me" is a LOP on the alu pipe where
+            //  lane == __ffs(peers) - 1 cost a BREV + FLO on the quarter-rate XU pipe)
+            if ((peers & lt) == 0) atomicAdd(counts + b, (u32)__popc(peers));
             if (++cx > b1x) {
                 cx = b0x;
                 if (++cy > b1y) {
@@ -261,8 +263,8 @@ __global__ void __launch_bounds__(256) k3_scatter(Params p, const uint2* __restr
         }
         // both groups' atomics in flight before either result is used
         u32 baseA = 0, baseB = 0;
-        if (peersA && lane == __ffs(peersA) - 1) baseA = atomicAdd(cursor + bA, (u32)__popc(peersA));
-        if (peersB && lane == __ffs(peersB) - 1) baseB = atomicAdd(cursor + bB, (u32)__popc(peersB));
+        if (peersA && (peersA & lt) == 0) baseA = atomicAdd(cursor + bA, (u32)__popc(peersA));
+        if (peersB && (peersB & lt) == 0) baseB = atomicAdd(cursor + bB, (u32)__popc(peersB));
         if (peersA) {
             baseA = __shfl_sync(peersA, baseA, __ffs(peersA) - 1);
             const u32 pos = baseA + (u32)__popc(peersA & lt);
