@@ -19,7 +19,8 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 SUBSET = ("small_configs or sparse_output or ragged or oversized or max_extent or straddle or randomized_jobs or "
           "unit_and_zero or random_soup or all_tets_culled or empty_mesh or p1_single or pipe_stream or "
           "gpu_lattice_input_matches or lattice_through_the_pipe or batched_lattice or fit_test or more_meshes or "
-          "random_lattices or huge_index or graph_replay")
+          "random_lattices or huge_index or graph_replay or swept_across or default_path_of_lattice or "
+          "two_calls_in_a_row or built_in_workspace")
 
 
 def _checked_lib():
@@ -33,7 +34,7 @@ def test_parity_subset_under_the_checked_build():
     code = (
         "import json, sys, pytest\n"
         f"rc = pytest.main(['-q', '-x', '-m', 'gpu', '-p', 'no:cacheprovider', '-k', {SUBSET!r}, "
-        "'tests/test_gpu_parity.py', 'tests/test_lattice.py'])\n"
+        "'tests/test_gpu_parity.py', 'tests/test_lattice.py', 'tests/test_zz_no_alloc.py'])\n"
         "import paper_2106_01326_b200 as pkg\n"
         "compiled, check = pkg.debug_check_status()\n"
         "print('CHECKED_RESULT ' + json.dumps({'rc': int(rc), 'compiled': compiled, 'check': check, 'lib': pkg.lib_path()}))\n"
